@@ -1,0 +1,678 @@
+/*
+ * floodped_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see floodped_oracle.h).
+ *
+ * One coupled step n -> n+1 (S:8c "O1..O5"), every read at level n (the paper's
+ * "simultaneous" update):
+ *   O1 occupancy N_p -> roughness
+ *   O2 flood cells, Eq. (2)
+ *   O3 pedestrians
+ *   O4 sandbag barrier -> z
+ *   O5 t += dt ; CFL dt for the next step P:L174
+ *
+ * Everything is double.  When real_bits == 32 the handful of expressions that
+ * decide an INTEGER output (cell index, risk state, timer expiry) are rounded to
+ * float after every single operation through rnd(): for + - * / on float inputs,
+ * double arithmetic followed by one rounding to float equals the float operation
+ * (53 >= 2*24+2), so both sides take those decisions in the same precision.
+ *
+ * No blocking, fusion or reordering: loops over cells, faces and agents as written.
+ */
+#include "floodped_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+struct orc_sim {
+    orc_config c;                 /* scalar copy; pointers below are owned copies */
+    int ncell;
+    double *z, *n0, *h, *qx, *qy, *h1, *qx1, *qy1;
+    unsigned char *mask;
+    int *Np;
+    int *inflow_mult[4];          /* per side, how many listed inflow faces sit on that cell side */
+    double inflow_length;         /* total length of all inflow faces */
+    int *inflow_cell; unsigned char *inflow_side;
+    double *hydro_t, *hydro_q;
+    unsigned char *nav_dir;
+    int *exit_cells, *line_cells;
+    /* pedestrians */
+    int np;
+    double *x, *y, *vx, *vy, *vpref, *timer;
+    double *x1, *y1, *vx1, *vy1, *timer1;
+    unsigned char *role, *state, *fsm, *active, *state1, *fsm1, *active1;
+    int *cell;                    /* level-n cell of each agent in the most recent step */
+    /* cell list */
+    int kbin, nbx, nby;
+    int *head, *next;
+    /* scalars */
+    double t, dt;
+    long long step, deposits, neg_clamps;
+    double clamped_volume;
+    int cursor, layer, bags, complete;
+};
+
+static double rnd(const orc_sim *s, double v) { return s->c.real_bits == 32 ? (double)(float)v : v; }
+static double rnd_bits(int real_bits, double v) { return real_bits == 32 ? (double)(float)v : v; }
+
+/* ------------------------------------------------------------------ building blocks */
+
+void orc_riemann_flux(double g, double hL, double unL, double utL,
+                      double hR, double unR, double utR, double F[3])
+{
+    /* S:8c-O2.1: both dry -> 0 */
+    if (hL <= 0.0 && hR <= 0.0) { F[0] = F[1] = F[2] = 0.0; return; }
+    double cL = sqrt(g * hL), cR = sqrt(g * hR);
+    double sL, sR;
+    if (hL <= 0.0) {                       /* dry on the left */
+        sL = unR - 2.0 * cR; sR = unR + cR;
+    } else if (hR <= 0.0) {                /* dry on the right */
+        sL = unL - cL; sR = unL + 2.0 * cL;
+    } else {                               /* two-rarefaction estimates (S:8c-C3) */
+        double us = 0.5 * (unL + unR) + cL - cR;
+        double cs = 0.5 * (cL + cR) + 0.25 * (unL - unR);
+        sL = fmin(unL - cL, us - cs);
+        sR = fmax(unR + cR, us + cs);
+    }
+    /* physical fluxes F = (h u, h u^2 + g h^2/2, .) */
+    double FL0 = hL * unL, FL1 = hL * unL * unL + 0.5 * g * hL * hL;
+    double FR0 = hR * unR, FR1 = hR * unR * unR + 0.5 * g * hR * hR;
+    if (sL >= 0.0)      { F[0] = FL0; F[1] = FL1; }
+    else if (sR <= 0.0) { F[0] = FR0; F[1] = FR1; }
+    else {
+        F[0] = (sR * FL0 - sL * FR0 + sL * sR * (hR - hL)) / (sR - sL);
+        F[1] = (sR * FL1 - sL * FR1 + sL * sR * (hR * unR - hL * unL)) / (sR - sL);
+    }
+    /* contact wave: tangential momentum is advected by the mass flux */
+    double num = sL * hR * (unR - sR) - sR * hL * (unL - sL);
+    double den = hR * (unR - sR) - hL * (unL - sL);
+    double sM = (den == 0.0) ? 0.0 : num / den;
+    F[2] = F[0] * (sM >= 0.0 ? utL : utR);
+}
+
+void orc_face(double g, double hi, double uni, double uti, double zi,
+              double hk, double unk, double utk, double zk,
+              double F[3], double *Fn_i, double *Fn_k)
+{
+    /* hydrostatic reconstruction (S:8c-C4; the "terrain integration and wetting-and-drying
+     * treatment" of P:L108): face bed = max, depths cut at the face bed, velocities kept */
+    double zf = fmax(zi, zk);
+    double his = fmax(0.0, (hi + zi) - zf);
+    double hks = fmax(0.0, (hk + zk) - zf);
+    orc_riemann_flux(g, his, uni, uti, hks, unk, utk, F);
+    /* bed-slope source folded into the face: each side sees F[1] - g h*^2/2 */
+    *Fn_i = F[1] - 0.5 * g * his * his;
+    *Fn_k = F[1] - 0.5 * g * hks * hks;
+}
+
+void orc_friction(double g, double n, double dt, double h_dry, double h, double *qx, double *qy)
+{
+    if (h > h_dry) {
+        double D = 1.0 + dt * g * n * n * sqrt((*qx) * (*qx) + (*qy) * (*qy)) / pow(h, 7.0 / 3.0);
+        *qx /= D; *qy /= D;
+    } else { *qx = 0.0; *qy = 0.0; }
+}
+
+double orc_cell_dt(double g, double cfl, double dx, double dy, double h, double u, double v)
+{
+    double c = sqrt(g * h);
+    return cfl * fmin(dx / (fabs(u) + c), dy / (fabs(v) + c));
+}
+
+double orc_hazard_rate(int real_bits, double h, double u, double v)
+{
+    double V = fmax(fabs(u), fabs(v));
+    return rnd_bits(real_bits, rnd_bits(real_bits, V + 0.5) * h);
+}
+
+int orc_risk_state(int real_bits, double h, double hr, double h_dry, const double e[4])
+{
+    if (!(h > rnd_bits(real_bits, h_dry))) return ORC_DRY;   /* S:8c-C17 */
+    if (hr < rnd_bits(real_bits, e[0])) return ORC_LOW;      /* half-open [lo,hi) */
+    if (hr < rnd_bits(real_bits, e[1])) return ORC_MEDIUM;
+    if (hr < rnd_bits(real_bits, e[2])) return ORC_HIGH;
+    return ORC_HIGHEST;
+}
+
+double orc_roughness(double n0, int Np, int cap)
+{
+    int m = Np < cap ? Np : cap;
+    return n0 * (1.0 + (double)m);                           /* n_M + N_p n_M */
+}
+
+double orc_hydrograph(int n, const double *t, const double *q, double time)
+{
+    if (n <= 0) return 0.0;
+    if (time <= t[0]) return q[0];
+    for (int k = 0; k + 1 < n; ++k)
+        if (time < t[k + 1])
+            return q[k] + (q[k + 1] - q[k]) * (time - t[k]) / (t[k + 1] - t[k]);
+    return q[n - 1];
+}
+
+static void pair_accel(double A_s, double B_s, double radius, double R_int,
+                       double xi, double yi, double xj, double yj, double *ax, double *ay)
+{
+    double ddx = xi - xj, ddy = yi - yj;
+    double d = sqrt(ddx * ddx + ddy * ddy);
+    if (d > 0.0 && d < R_int) {                              /* S:8c-O3.4, C26 */
+        double f = A_s * exp((2.0 * radius - d) / B_s);
+        *ax += f * ddx / d; *ay += f * ddy / d;
+    }
+}
+
+void orc_social_bruteforce(int n, const double *x, const double *y, const unsigned char *active,
+                           double A_s, double B_s, double radius, double R_int,
+                           int i, double *ax, double *ay)
+{
+    *ax = 0.0; *ay = 0.0;
+    for (int j = 0; j < n; ++j)
+        if (j != i && active[j]) pair_accel(A_s, B_s, radius, R_int, x[i], y[i], x[j], y[j], ax, ay);
+}
+
+/* ------------------------------------------------------------------ helpers */
+
+static void *dup_mem(const void *p, size_t bytes)
+{
+    void *q = malloc(bytes ? bytes : 1);
+    if (p && bytes) memcpy(q, p, bytes); else memset(q, 0, bytes ? bytes : 1);
+    return q;
+}
+
+static int cell_ix(const orc_sim *s, double x)
+{
+    double inv = rnd(s, 1.0 / s->c.dx);
+    int i = (int)floor(rnd(s, x * inv));
+    if (i < 0) i = 0;
+    if (i > s->c.nx - 1) i = s->c.nx - 1;
+    return i;
+}
+static int cell_iy(const orc_sim *s, double y)
+{
+    double inv = rnd(s, 1.0 / s->c.dy);
+    int j = (int)floor(rnd(s, y * inv));
+    if (j < 0) j = 0;
+    if (j > s->c.ny - 1) j = s->c.ny - 1;
+    return j;
+}
+/* is the point outside the domain or in a solid cell? (move rejection, S:8c-O3.6) */
+static int blocked(const orc_sim *s, double x, double y)
+{
+    double fi = floor(rnd(s, x * rnd(s, 1.0 / s->c.dx)));
+    double fj = floor(rnd(s, y * rnd(s, 1.0 / s->c.dy)));
+    if (fi < 0.0 || fi >= (double)s->c.nx || fj < 0.0 || fj >= (double)s->c.ny) return 1;
+    return s->mask[(int)fj * s->c.nx + (int)fi] != 0;
+}
+
+static int cheb(const orc_sim *s, int ca, int cb)
+{
+    int ai = ca % s->c.nx, aj = ca / s->c.nx, bi = cb % s->c.nx, bj = cb / s->c.nx;
+    int di = abs(ai - bi), dj = abs(aj - bj);
+    return di > dj ? di : dj;
+}
+
+static void velocity_of(const orc_sim *s, double h, double qx, double qy, double *u, double *v)
+{
+    if (h > s->c.h_dry) { *u = qx / h; *v = qy / h; } else { *u = 0.0; *v = 0.0; }
+}
+
+static double next_dt(const orc_sim *s, const double *h, const double *qx, const double *qy)
+{
+    /* S:8c-O5: CFL over wet cells, capped by dt_max which is also the dry value */
+    double dt = s->c.dt_max;
+    for (int c = 0; c < s->ncell; ++c) {
+        if (s->mask[c] || !(h[c] > s->c.h_dry)) continue;
+        double u, v; velocity_of(s, h[c], qx[c], qy[c], &u, &v);
+        double d = orc_cell_dt(s->c.g, s->c.cfl, s->c.dx, s->c.dy, h[c], u, v);
+        if (d < dt) dt = d;
+    }
+    return dt;
+}
+
+static void build_cell_list(orc_sim *s)
+{
+    int nb = s->nbx * s->nby;
+    for (int b = 0; b < nb; ++b) s->head[b] = -1;
+    /* insert in reverse so that each list is in increasing agent index */
+    for (int i = s->np - 1; i >= 0; --i) {
+        if (!s->active[i]) continue;
+        int b = (cell_iy(s, s->y[i]) / s->kbin) * s->nbx + cell_ix(s, s->x[i]) / s->kbin;
+        s->next[i] = s->head[b]; s->head[b] = i;
+    }
+}
+
+static void social_from_list(const orc_sim *s, int i, double *ax, double *ay)
+{
+    *ax = 0.0; *ay = 0.0;
+    int bx = cell_ix(s, s->x[i]) / s->kbin, by = cell_iy(s, s->y[i]) / s->kbin;
+    for (int jy = by - 1; jy <= by + 1; ++jy)
+        for (int jx = bx - 1; jx <= bx + 1; ++jx) {
+            if (jx < 0 || jy < 0 || jx >= s->nbx || jy >= s->nby) continue;
+            for (int j = s->head[jy * s->nbx + jx]; j >= 0; j = s->next[j])
+                if (j != i)
+                    pair_accel(s->c.A_s, s->c.B_s, s->c.radius, s->c.R_int,
+                               s->x[i], s->y[i], s->x[j], s->y[j], ax, ay);
+        }
+}
+
+/* ------------------------------------------------------------------ create / destroy */
+
+orc_sim *orc_create(const orc_config *cfg)
+{
+    if (!cfg || cfg->nx <= 0 || cfg->ny <= 0 || !(cfg->dx > 0) || !(cfg->dy > 0)) return NULL;
+    orc_sim *s = (orc_sim *)calloc(1, sizeof *s);
+    s->c = *cfg;
+    int nc = s->ncell = cfg->nx * cfg->ny;
+    size_t nb = (size_t)nc * sizeof(double);
+    s->z = dup_mem(cfg->z, nb);
+    s->n0 = dup_mem(cfg->manning, nb);
+    s->mask = dup_mem(cfg->mask, (size_t)nc);
+    s->h = dup_mem(cfg->h0, nb);
+    s->qx = dup_mem(NULL, nb); s->qy = dup_mem(NULL, nb);
+    s->h1 = dup_mem(NULL, nb); s->qx1 = dup_mem(NULL, nb); s->qy1 = dup_mem(NULL, nb);
+    for (int c = 0; c < nc; ++c) {
+        if (s->mask[c]) { s->h[c] = 0.0; continue; }
+        s->qx[c] = s->h[c] * (cfg->u0 ? cfg->u0[c] : 0.0);   /* store conserved (S:8c-C8) */
+        s->qy[c] = s->h[c] * (cfg->v0 ? cfg->v0[c] : 0.0);
+    }
+    s->Np = dup_mem(NULL, (size_t)nc * sizeof(int));
+    s->inflow_length = 0.0;
+    for (int k = 0; k < 4; ++k) s->inflow_mult[k] = dup_mem(NULL, (size_t)nc * sizeof(int));
+    for (int f = 0; f < cfg->n_inflow; ++f) {
+        int side = cfg->inflow_side[f];
+        s->inflow_mult[side][cfg->inflow_cell[f]] += 1;
+        s->inflow_length += (side == ORC_W || side == ORC_E) ? cfg->dy : cfg->dx;
+    }
+    s->inflow_cell = dup_mem(cfg->inflow_cell, (size_t)cfg->n_inflow * sizeof(int));
+    s->inflow_side = dup_mem(cfg->inflow_side, (size_t)cfg->n_inflow);
+    s->hydro_t = dup_mem(cfg->hydro_t, (size_t)cfg->n_hydro * sizeof(double));
+    s->hydro_q = dup_mem(cfg->hydro_q, (size_t)cfg->n_hydro * sizeof(double));
+    s->nav_dir = dup_mem(cfg->nav_dir, (size_t)cfg->n_targets * (size_t)nc);
+    s->exit_cells = dup_mem(cfg->exit_cells, (size_t)cfg->n_exit_cells * sizeof(int));
+    s->line_cells = dup_mem(cfg->line_cells, (size_t)cfg->n_line * sizeof(int));
+
+    int np = s->np = cfg->n_peds;
+    size_t pb = (size_t)np * sizeof(double);
+    s->x = dup_mem(cfg->px, pb); s->y = dup_mem(cfg->py, pb);
+    s->vx = dup_mem(cfg->pvx, pb); s->vy = dup_mem(cfg->pvy, pb);
+    s->vpref = dup_mem(cfg->pvpref, pb);
+    s->timer = dup_mem(NULL, pb);
+    s->x1 = dup_mem(NULL, pb); s->y1 = dup_mem(NULL, pb);
+    s->vx1 = dup_mem(NULL, pb); s->vy1 = dup_mem(NULL, pb); s->timer1 = dup_mem(NULL, pb);
+    s->role = dup_mem(cfg->prole, (size_t)np);
+    s->state = dup_mem(NULL, (size_t)np); s->state1 = dup_mem(NULL, (size_t)np);
+    s->fsm = dup_mem(NULL, (size_t)np); s->fsm1 = dup_mem(NULL, (size_t)np);
+    s->active = dup_mem(NULL, (size_t)np); s->active1 = dup_mem(NULL, (size_t)np);
+    s->cell = dup_mem(NULL, (size_t)np * sizeof(int));
+    for (int i = 0; i < np; ++i) {
+        s->active[i] = 1;
+        s->fsm[i] = s->role[i] ? ORC_TO_STORAGE : ORC_EVACUATE;
+        s->cell[i] = cell_iy(s, s->y[i]) * cfg->nx + cell_ix(s, s->x[i]);
+    }
+    /* default cap so that nobody crosses more than one cell per step (S:8c-C10) */
+    if (!(s->c.dt_max > 0.0)) {
+        double vm = 1.8;
+        for (int i = 0; i < np; ++i) if (s->vpref[i] > vm) vm = s->vpref[i];
+        for (int k = 0; k < 4; ++k) if (cfg->speed_wet[k] > vm) vm = cfg->speed_wet[k];
+        double dmin = cfg->dx < cfg->dy ? cfg->dx : cfg->dy;
+        s->c.dt_max = fmin(1.0, dmin / (cfg->vmax_factor * vm));
+    }
+    /* sort bins: k x k cells with k dx >= R_int so that 3x3 bins are complete (S:8c-C26) */
+    {
+        double dmin = cfg->dx < cfg->dy ? cfg->dx : cfg->dy;
+        s->kbin = (int)ceil(cfg->R_int / dmin);
+        if (s->kbin < 1) s->kbin = 1;
+        s->nbx = (cfg->nx + s->kbin - 1) / s->kbin;
+        s->nby = (cfg->ny + s->kbin - 1) / s->kbin;
+        s->head = dup_mem(NULL, (size_t)s->nbx * s->nby * sizeof(int));
+        s->next = dup_mem(NULL, (size_t)np * sizeof(int));
+    }
+    s->t = 0.0; s->step = 0;
+    s->complete = (cfg->n_line <= 0 || cfg->n_layers <= 0) ? 1 : 0;
+    s->dt = next_dt(s, s->h, s->qx, s->qy);
+    if (s->t + s->dt > s->c.t_end) s->dt = fmax(0.0, s->c.t_end - s->t);
+    return s;
+}
+
+void orc_destroy(orc_sim *s)
+{
+    if (!s) return;
+    void *p[] = { s->z, s->n0, s->h, s->qx, s->qy, s->h1, s->qx1, s->qy1, s->mask, s->Np,
+        s->inflow_mult[0], s->inflow_mult[1], s->inflow_mult[2], s->inflow_mult[3],
+        s->inflow_cell, s->inflow_side, s->hydro_t, s->hydro_q, s->nav_dir, s->exit_cells,
+        s->line_cells, s->x, s->y, s->vx, s->vy, s->vpref, s->timer, s->x1, s->y1, s->vx1, s->vy1,
+        s->timer1, s->role, s->state, s->fsm, s->active, s->state1, s->fsm1, s->active1, s->cell,
+        s->head, s->next };
+    for (size_t k = 0; k < sizeof p / sizeof p[0]; ++k) free(p[k]);
+    free(s);
+}
+
+/* ------------------------------------------------------------------ one coupled step */
+
+/* state of the neighbour across one face of cell c: the cell itself if it is an interior
+ * walkable cell, else the wall ghost (S:8c-O2.1): same h and z, normal velocity
+ * negated, tangential kept */
+static void neighbour(const orc_sim *s, int c, int i, int j, int di, int dj,
+                      double hc, double unc, double utc, double zc,
+                      double *hk, double *unk, double *utk, double *zk)
+{
+    int ii = i + di, jj = j + dj;
+    int wall = (ii < 0 || jj < 0 || ii >= s->c.nx || jj >= s->c.ny);
+    int k = wall ? c : jj * s->c.nx + ii;
+    if (!wall && s->mask[k]) wall = 1;
+    if (wall) { *hk = hc; *unk = -unc; *utk = utc; *zk = zc; return; }
+    double u, v; velocity_of(s, s->h[k], s->qx[k], s->qy[k], &u, &v);
+    *hk = s->h[k]; *zk = s->z[k];
+    if (di != 0) { *unk = u; *utk = v; } else { *unk = v; *utk = u; }
+}
+
+static void flood_step(orc_sim *s, double q_in)
+{
+    const double g = s->c.g, dt = s->dt, dx = s->c.dx, dy = s->c.dy;
+    const int nx = s->c.nx, ny = s->c.ny;
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            int c = j * nx + i;
+            if (s->mask[c]) { s->h1[c] = s->qx1[c] = s->qy1[c] = 0.0; continue; }   /* S:8c-C16 */
+            double h = s->h[c], z = s->z[c], u, v;
+            velocity_of(s, h, s->qx[c], s->qy[c], &u, &v);
+            double hk, unk, utk, zk, F[3], Fi, Fk;
+
+            /* EAST: cell is the left state; normal u, tangential v */
+            neighbour(s, c, i, j, +1, 0, h, u, v, z, &hk, &unk, &utk, &zk);
+            orc_face(g, h, u, v, z, hk, unk, utk, zk, F, &Fi, &Fk);
+            double FE0 = F[0], FE1 = Fi, FE2 = F[2];
+            /* WEST: cell is the right state */
+            neighbour(s, c, i, j, -1, 0, h, u, v, z, &hk, &unk, &utk, &zk);
+            orc_face(g, hk, unk, utk, zk, h, u, v, z, F, &Fk, &Fi);
+            double FW0 = F[0], FW1 = Fi, FW2 = F[2];
+            /* NORTH: cell is the lower state; normal v, tangential u */
+            neighbour(s, c, i, j, 0, +1, h, v, u, z, &hk, &unk, &utk, &zk);
+            orc_face(g, h, v, u, z, hk, unk, utk, zk, F, &Fi, &Fk);
+            double GN0 = F[0], GN2 = Fi, GN1 = F[2];
+            /* SOUTH: cell is the upper state */
+            neighbour(s, c, i, j, 0, -1, h, v, u, z, &hk, &unk, &utk, &zk);
+            orc_face(g, hk, unk, utk, zk, h, v, u, z, F, &Fk, &Fi);
+            double GS0 = F[0], GS2 = Fi, GS1 = F[2];
+
+            /* inflow faces: wall for momentum, prescribed mass flux into the domain
+             * (S:8c-O2.1, C14) */
+            FW0 += q_in * s->inflow_mult[ORC_W][c];
+            FE0 -= q_in * s->inflow_mult[ORC_E][c];
+            GS0 += q_in * s->inflow_mult[ORC_S][c];
+            GN0 -= q_in * s->inflow_mult[ORC_N][c];
+
+            /* Eq. (2) */
+            double hn  = h        - dt / dx * (FE0 - FW0) - dt / dy * (GN0 - GS0);
+            double qxn = s->qx[c] - dt / dx * (FE1 - FW1) - dt / dy * (GN1 - GS1);
+            double qyn = s->qy[c] - dt / dx * (FE2 - FW2) - dt / dy * (GN2 - GS2);
+            /* accounted clamp (S:8c-C12) */
+            if (hn < 0.0) { s->clamped_volume += -hn * dx * dy; s->neg_clamps += 1; hn = 0.0; }
+            /* Manning friction with the occupancy-dependent roughness */
+            double n = s->c.couple_roughness ? orc_roughness(s->n0[c], s->Np[c], s->c.n_cap) : s->n0[c];
+            orc_friction(g, n, dt, s->c.h_dry, hn, &qxn, &qyn);
+            s->h1[c] = hn; s->qx1[c] = qxn; s->qy1[c] = qyn;
+        }
+}
+
+static void dir_vector(int code, double *ex, double *ey)
+{
+    static const double r = 0.70710678118654752440;
+    switch (code) {
+    case 0: *ex = 1;  *ey = 0;  break;   case 1: *ex = r;  *ey = r;  break;
+    case 2: *ex = 0;  *ey = 1;  break;   case 3: *ex = -r; *ey = r;  break;
+    case 4: *ex = -1; *ey = 0;  break;   case 5: *ex = -r; *ey = -r; break;
+    case 6: *ex = 0;  *ey = -1; break;   case 7: *ex = r;  *ey = -r; break;
+    default: *ex = 0; *ey = 0;
+    }
+}
+
+/* returns number of deposit events D */
+static long long ped_step(orc_sim *s)
+{
+    const orc_config *p = &s->c;
+    const double dt = s->dt;
+    const int complete0 = s->complete;           /* value at the start of the step (S:8c-O3.7) */
+    long long D = 0;
+    build_cell_list(s);
+    for (int i = 0; i < s->np; ++i) {
+        s->x1[i] = s->x[i]; s->y1[i] = s->y[i]; s->vx1[i] = s->vx[i]; s->vy1[i] = s->vy[i];
+        s->timer1[i] = s->timer[i]; s->state1[i] = s->state[i]; s->fsm1[i] = s->fsm[i];
+        s->active1[i] = s->active[i];
+        if (!s->active[i]) continue;
+        /* 1. containing cell, sample U^n there (S:8c-C19, C20) */
+        int c = s->cell[i];
+        int fsm = s->fsm[i];
+        /* 8. exit (S:8c-C29): evaluated on the level-n cell */
+        if (s->role[i] == 0 || fsm == ORC_EVACUATE) {
+            int out = 0;
+            for (int e = 0; e < p->n_exit_cells; ++e)
+                if (cheb(s, c, s->exit_cells[e]) <= p->arrive_cells) out = 1;
+            if (out) { s->active1[i] = 0; continue; }
+        }
+        double h = s->h[c], u, v;
+        if (h > rnd(s, p->h_dry)) { u = rnd(s, s->qx[c] / h); v = rnd(s, s->qy[c] / h); }
+        else { u = 0.0; v = 0.0; }
+        double hr = orc_hazard_rate(p->real_bits, h, u, v);
+        int st = orc_risk_state(p->real_bits, h, hr, p->h_dry, p->hr_edges);  /* Table 1 */
+        s->state1[i] = (unsigned char)st;
+        /* 2. desired speed (S:8c-C18) */
+        double v0 = (st == ORC_DRY) ? s->vpref[i] : p->speed_wet[st - 1];
+        if (fsm == ORC_PICKING || fsm == ORC_DROPPING) v0 = 0.0;              /* waiting */
+        /* 3. target field by role / FSM */
+        int target = p->exit_target;
+        if (fsm == ORC_TO_STORAGE) target = p->storage_target;
+        else if (fsm == ORC_TO_BARRIER) target = p->drop_target;
+        double ex, ey;
+        dir_vector(s->nav_dir[(size_t)target * s->ncell + c], &ex, &ey);
+        /* 4. social repulsion from agents in adjacent bins (S:8c-C24, C26) */
+        double ax, ay;
+        social_from_list(s, i, &ax, &ay);
+        /* 5. velocity: backward Euler on the relaxation term (S:8c-C25) */
+        double wx = (s->vx[i] + dt * (v0 * ex / p->tau + ax)) / (1.0 + dt / p->tau);
+        double wy = (s->vy[i] + dt * (v0 * ey / p->tau + ay)) / (1.0 + dt / p->tau);
+        double wmax = p->vmax_factor * v0, wn = sqrt(wx * wx + wy * wy);
+        if (wn > wmax) { double f = (wn > 0.0) ? wmax / wn : 0.0; wx *= f; wy *= f; }
+        /* 6. position with axis-separated rejection at walls and solids (S:8c-C27) */
+        double xn = s->x[i] + dt * wx, yn = s->y[i];
+        if (blocked(s, xn, yn)) { xn = s->x[i]; wx = 0.0; }
+        yn = s->y[i] + dt * wy;
+        if (blocked(s, xn, yn)) { yn = s->y[i]; wy = 0.0; }
+        s->x1[i] = xn; s->y1[i] = yn; s->vx1[i] = wx; s->vy1[i] = wy;
+        /* 7. responder FSM on the level-n cell, once per step (S:8c-C31) */
+        if (s->role[i] == 1) {
+            if (fsm == ORC_TO_STORAGE) {
+                if (cheb(s, c, p->storage_cell) <= p->arrive_cells) { s->fsm1[i] = ORC_PICKING; s->timer1[i] = rnd(s, p->t_pick); }
+            } else if (fsm == ORC_PICKING) {
+                s->timer1[i] = rnd(s, s->timer[i] - rnd(s, dt));
+                if (s->timer1[i] <= 0.0) s->fsm1[i] = ORC_TO_BARRIER;
+            } else if (fsm == ORC_TO_BARRIER) {
+                if (cheb(s, c, p->drop_cell) <= p->arrive_cells) { s->fsm1[i] = ORC_DROPPING; s->timer1[i] = rnd(s, p->t_drop); }
+            } else if (fsm == ORC_DROPPING) {
+                s->timer1[i] = rnd(s, s->timer[i] - rnd(s, dt));
+                if (s->timer1[i] <= 0.0) { D += 1; s->fsm1[i] = complete0 ? ORC_EVACUATE : ORC_TO_STORAGE; }
+            }
+        }
+    }
+    return D;
+}
+
+static void barrier_step(orc_sim *s, long long D)
+{
+    /* gather bags until one layer covers the cell, raise z by one bag thickness,
+     * move to the next cell of the line, repeat N_L layers (S:8c-O4, C33, C34) */
+    s->deposits += D;
+    for (long long d = 0; d < D; ++d) {
+        if (s->complete) break;
+        s->bags += 1;
+        if (s->bags == s->c.bags_per_cell_layer) {
+            s->z[s->line_cells[s->cursor]] += s->c.layer_thickness;
+            s->bags = 0; s->cursor += 1;
+            if (s->cursor == s->c.n_line) { s->layer += 1; s->cursor = 0; }
+            if (s->layer == s->c.n_layers) s->complete = 1;
+        }
+    }
+}
+
+int orc_step(orc_sim *s, long long n)
+{
+    for (long long k = 0; k < n; ++k) {
+        if (s->t >= s->c.t_end) break;                      /* no-op once t_end is reached */
+        /* O1 */
+        memset(s->Np, 0, (size_t)s->ncell * sizeof(int));
+        for (int i = 0; i < s->np; ++i) {
+            if (!s->active[i]) continue;
+            s->cell[i] = cell_iy(s, s->y[i]) * s->c.nx + cell_ix(s, s->x[i]);
+            s->Np[s->cell[i]] += 1;                         /* all active pedestrians (S:8c-C21) */
+        }
+        /* O2 */
+        double Q = orc_hydrograph(s->c.n_hydro, s->hydro_t, s->hydro_q, s->t);
+        double q_in = (s->inflow_length > 0.0) ? Q / s->inflow_length : 0.0;
+        flood_step(s, q_in);
+        /* O3 (reads level-n flood and pedestrians) */
+        long long D = ped_step(s);
+        /* O4 */
+        barrier_step(s, D);
+        /* commit level n+1 */
+        double *tp;
+#define SWAP(a, b) do { tp = a; a = b; b = tp; } while (0)
+        SWAP(s->h, s->h1); SWAP(s->qx, s->qx1); SWAP(s->qy, s->qy1);
+        SWAP(s->x, s->x1); SWAP(s->y, s->y1); SWAP(s->vx, s->vx1); SWAP(s->vy, s->vy1);
+        SWAP(s->timer, s->timer1);
+#undef SWAP
+        unsigned char *tb;
+        tb = s->state; s->state = s->state1; s->state1 = tb;
+        tb = s->fsm; s->fsm = s->fsm1; s->fsm1 = tb;
+        tb = s->active; s->active = s->active1; s->active1 = tb;
+        /* O5 */
+        s->t += s->dt;
+        s->step += 1;
+        s->dt = next_dt(s, s->h, s->qx, s->qy);
+        if (s->t + s->dt > s->c.t_end) s->dt = fmax(0.0, s->c.t_end - s->t);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ read / write */
+
+void orc_get_stats(orc_sim *s, orc_stats *o)
+{
+    memset(o, 0, sizeof *o);
+    o->t = s->t; o->dt = s->dt; o->step = s->step;
+    double comp = 0.0;                       /* compensated (Neumaier) sum of the volume */
+    for (int c = 0; c < s->ncell; ++c) {
+        if (s->mask[c]) continue;
+        double u, v; velocity_of(s, s->h[c], s->qx[c], s->qy[c], &u, &v);
+        double hr = (s->h[c] > s->c.h_dry) ? orc_hazard_rate(64, s->h[c], u, v) : 0.0;
+        double term = s->h[c] * s->c.dx * s->c.dy, tsum = o->volume + term;
+        comp += (fabs(o->volume) >= fabs(term)) ? (o->volume - tsum) + term : (term - tsum) + o->volume;
+        o->volume = tsum;
+        if (s->h[c] > o->max_h) o->max_h = s->h[c];
+        if (hr > o->max_hr) o->max_hr = hr;
+    }
+    o->volume += comp;
+    for (int i = 0; i < s->np; ++i) o->hist[s->active[i] ? s->state[i] : 5] += 1;
+    o->neg_depth_clamps = s->neg_clamps; o->clamped_volume = s->clamped_volume;
+    o->cursor = s->cursor; o->layer = s->layer; o->bags = s->bags;
+    o->barrier_complete = s->complete; o->deposits = s->deposits;
+}
+
+void orc_read_flood(orc_sim *s, double *h, double *u, double *v, double *z, double *hr)
+{
+    for (int c = 0; c < s->ncell; ++c) {
+        double uu, vv; velocity_of(s, s->h[c], s->qx[c], s->qy[c], &uu, &vv);
+        if (h) h[c] = s->h[c];
+        if (u) u[c] = uu;
+        if (v) v[c] = vv;
+        if (z) z[c] = s->z[c];
+        if (hr) hr[c] = (s->h[c] > s->c.h_dry) ? orc_hazard_rate(64, s->h[c], uu, vv) : 0.0;
+    }
+}
+
+void orc_read_conserved(orc_sim *s, double *h, double *qx, double *qy)
+{
+    size_t nb = (size_t)s->ncell * sizeof(double);
+    if (h) memcpy(h, s->h, nb);
+    if (qx) memcpy(qx, s->qx, nb);
+    if (qy) memcpy(qy, s->qy, nb);
+}
+
+void orc_read_occupancy(orc_sim *s, int *Np) { memcpy(Np, s->Np, (size_t)s->ncell * sizeof(int)); }
+
+void orc_read_peds(orc_sim *s, double *x, double *y, double *vx, double *vy,
+                   unsigned char *state, unsigned char *fsm, unsigned char *active,
+                   int *cell, double *timer)
+{
+    for (int i = 0; i < s->np; ++i) {
+        if (x) x[i] = s->x[i];
+        if (y) y[i] = s->y[i];
+        if (vx) vx[i] = s->vx[i];
+        if (vy) vy[i] = s->vy[i];
+        if (state) state[i] = s->state[i];
+        if (fsm) fsm[i] = s->fsm[i];
+        if (active) active[i] = s->active[i];
+        if (cell) cell[i] = cell_iy(s, s->y[i]) * s->c.nx + cell_ix(s, s->x[i]);
+        if (timer) timer[i] = s->timer[i];
+    }
+}
+
+void orc_social_celllist(orc_sim *s, double *ax, double *ay)
+{
+    build_cell_list(s);
+    for (int i = 0; i < s->np; ++i) {
+        ax[i] = ay[i] = 0.0;
+        if (s->active[i]) social_from_list(s, i, &ax[i], &ay[i]);
+    }
+}
+
+int orc_binning(orc_sim *s, int *key, int *count, int *start, int *nbx, int *nby, int *k)
+{
+    int nb = s->nbx * s->nby;
+    if (nbx) *nbx = s->nbx;
+    if (nby) *nby = s->nby;
+    if (k) *k = s->kbin;
+    if (count) memset(count, 0, (size_t)nb * sizeof(int));
+    for (int i = 0; i < s->np; ++i) {
+        int b = nb;                                           /* inactive agents sort last */
+        if (s->active[i])
+            b = (cell_iy(s, s->y[i]) / s->kbin) * s->nbx + cell_ix(s, s->x[i]) / s->kbin;
+        if (key) key[i] = b;
+        if (count && b < nb) count[b] += 1;
+    }
+    if (start && count) {
+        int acc = 0;
+        for (int b = 0; b < nb; ++b) { start[b] = acc; acc += count[b]; }
+        start[nb] = acc;
+    }
+    return nb;
+}
+
+void orc_write_flood(orc_sim *s, const double *h, const double *qx, const double *qy, const double *z)
+{
+    size_t nb = (size_t)s->ncell * sizeof(double);
+    if (h) memcpy(s->h, h, nb);
+    if (qx) memcpy(s->qx, qx, nb);
+    if (qy) memcpy(s->qy, qy, nb);
+    if (z) memcpy(s->z, z, nb);
+}
+
+void orc_write_peds(orc_sim *s, const double *x, const double *y, const double *vx, const double *vy,
+                    const unsigned char *fsm, const unsigned char *active, const double *timer)
+{
+    size_t pb = (size_t)s->np * sizeof(double);
+    if (x) memcpy(s->x, x, pb);
+    if (y) memcpy(s->y, y, pb);
+    if (vx) memcpy(s->vx, vx, pb);
+    if (vy) memcpy(s->vy, vy, pb);
+    if (fsm) memcpy(s->fsm, fsm, (size_t)s->np);
+    if (active) memcpy(s->active, active, (size_t)s->np);
+    if (timer) memcpy(s->timer, timer, pb);
+    for (int i = 0; i < s->np; ++i)
+        s->cell[i] = cell_iy(s, s->y[i]) * s->c.nx + cell_ix(s, s->x[i]);
+}
+
+void orc_set_time(orc_sim *s, double t, double dt) { s->t = t; s->dt = dt; }
+
+void orc_set_barrier(orc_sim *s, int cursor, int layer, int bags, int complete)
+{
+    s->cursor = cursor; s->layer = layer; s->bags = bags; s->complete = complete;
+}
