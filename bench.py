@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- coupled flood-pedestrian step on B200: one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+
+A "step" is ONE coupled step: occupancy -> binning (count, scan, scatter) -> pedestrian step ->
+flood step (+ CFL reduction) -> sandbag/time tail, over the whole synthetic workload.  Default
+workload: BASELINE.json configs[4] ("Throughput stress", 8192x8192 fp32 cells + 1e6 pedestrians,
+500 timed steps) -- the largest single-GPU configuration and the only one whose per-step traffic
+(2.3 GB) is larger than L2, which is what the "% of HBM roofline" part of the metric needs.
+
+value      = flood cell-updates/s of the whole job, inputs resident in HBM, CUDA graphs, CUDA events.
+e2e        = same metric through the C ABI with HOST (pinned) buffers: upload of the initial
+             state + K steps + read-back of depth/discharge/pedestrians inside the timed region.
+roofline   = flood kernel: algorithmic bytes per launch / its average duration (CUDA events around
+             each launch, sim_step_profiled) vs the measured HBM peak of MEASURED_PEAKS.json.
+cpu_baseline / --impl reference = the CPU oracle as it stands, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FLOOD_BYTES_PER_CELL = 33        # fp32: read h,qx,qy,z,n0 (20) + N_p (1) ; write h,qx,qy (12)  [DESIGN.md 6]
+PED_BYTES_PER_AGENT = 175        # key+count 17, scatter 72, step 85
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(self.index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            if ts < t0 - 0.05 or ts > t1 + 0.15:
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def scenario(cfg, small=False):
+    from paper_1908_05232_b200 import scenarios as S
+    if small:                       # CPU-oracle sample: same recipe, bounded size
+        kw = {1: {}, 2: {}, 3: {}, 4: dict(n=1024, n_peds=25_000), 5: dict(n=2048, n_peds=62_500)}[cfg]
+    else:
+        kw = {}
+    return S.make(cfg, **kw)
+
+
+def oracle_run(cfg, steps, warmup):
+    """The oracle as it stands, single thread, on the bounded sample; returns (cells/s, agents/s, s/step, desc)."""
+    import oracle
+    sc = scenario(cfg, small=True)
+    o = oracle.Oracle(sc)
+    if warmup:
+        o.step(warmup)
+    act0 = int((o.read_peds()["active"] == 1).sum()) if sc.n_peds else 0
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    done = o.stats()["step"] - warmup
+    desc = f"{sc.name} recipe at {sc.nx}x{sc.ny} cells, {sc.n_peds} pedestrians, {done} coupled steps after {warmup} warm-up"
+    return sc.nx * sc.ny * done / dt, act0 * done / dt, dt / max(done, 1), desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = min(args.steps, {1: 100, 2: 200, 3: 200, 4: 12, 5: 4}[args.config])
+    warm = min(args.warmup, 1)
+    cps, aps, sps, desc = oracle_run(args.config, steps, warm)
+    line = {
+        "impl": "reference", "metric": "flood cell-updates/s (coupled step)", "value": cps, "unit": "cell-updates/s",
+        "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * sps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "agent_updates_per_s": aps, "coupled_steps_per_s": 1.0 / sps,
+        "config": {"workload": f"config{args.config}", "sample": desc},
+        "cpu_baseline": {"value": cps, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": cps, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1908_05232_b200 import binding, build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    build.build()
+    K, W = args.steps, max(args.warmup, 3)
+    sc = scenario(args.config)
+    real = np.float32 if sc.real_bits == 32 else np.float64
+    ncell, npeds = sc.nx * sc.ny, sc.n_peds
+    g = binding.Sim(sc, device=f"cuda:{local}")
+    g.set_flood_variant(args.flood_variant if sc.nx % 4 == 0 else 0)
+    kps = g.kernels_per_step()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timed region (CUDA graphs)
+    g.step(W)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    st0 = g.stats()
+    barrier()
+    w0 = time.time()
+    e0.record()
+    g.step(K)
+    e1.record()
+    barrier()
+    w1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(w0, w1)
+    st1 = g.stats()
+    done = st1["step"] - st0["step"]
+    active = npeds - st0["hist"][5]
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+
+    # ---- per-kernel durations, CUDA events around every launch (same state, continuing)
+    KP = min(K, 100)
+    kms = g.step_profiled(KP)
+    flood_ms = kms["flood_step"] / KP
+    ped_ms = (kms["bin_count"] + kms["bin_scan"] + kms["scatter"] + kms["ped_step"]) / KP
+    peak, peak_src = peaks()
+    fb = FLOOD_BYTES_PER_CELL if sc.real_bits == 32 else 65
+    flood_gbs = ncell * fb / (flood_ms * 1e-3) / 1e9
+    kbin = int(np.ceil(sc.R_int / min(sc.dx, sc.dy)))
+    nbins = -(-sc.nx // kbin) * -(-sc.ny // kbin)
+    ped_gbs = (active * PED_BYTES_PER_AGENT + nbins * 12) / (ped_ms * 1e-3) / 1e9 if npeds else 0.0
+
+    # ---- end to end through the C ABI with pinned HOST buffers
+    host = {k: torch.empty(ncell, dtype=torch.float32 if real is np.float32 else torch.float64).pin_memory()
+            for k in ("h", "qx", "qy")}
+    c = g.read_conserved()
+    for k in host:
+        host[k].numpy()[:] = c[k]
+    p = g.read_peds()
+    pin = {k: torch.from_numpy(np.ascontiguousarray(p[k])).pin_memory() for k in ("x", "y", "vx", "vy", "timer", "fsm", "active")}
+    out_f = {k: torch.empty_like(host[k]).pin_memory() for k in host}
+    KE = min(K, 200)
+    h2d = 3 * ncell * host["h"].element_size() + sum(v.numel() * v.element_size() for v in pin.values())
+    d2h = 3 * ncell * host["h"].element_size() + npeds * (5 * host["h"].element_size() + 3 + 4)
+    barrier()
+    tt0 = time.perf_counter()
+    g.write_flood(host["h"].numpy(), host["qx"].numpy(), host["qy"].numpy())
+    if npeds:
+        g.write_peds(*(pin[k].numpy() for k in ("x", "y", "vx", "vy", "fsm", "active", "timer")))
+    g.set_time(st1["t"], st1["dt"])
+    g.step(KE)
+    g.read_conserved_into(out_f["h"].data_ptr(), out_f["qx"].data_ptr(), out_f["qy"].data_ptr())
+    pe = g.read_peds() if npeds else None
+    ste = g.stats()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - tt0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    e2e_done = KE
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- CPU oracle, bounded sample (reported baseline, not the target)
+    o_steps = {1: 100, 2: 100, 3: 100, 4: 8, 5: 4}[args.config]
+    if world == 1 and not args.no_cpu_baseline:
+        cps, aps, sps, desc = oracle_run(args.config, o_steps, 1)
+        cpu = {"value": cps, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": desc,
+               "agent_updates_per_s": aps}
+    else:
+        cpu = None
+
+    value = world * ncell * done / (ms_max * 1e-3)
+    line = {
+        "metric": "flood cell-updates/s (coupled step)", "value": value, "unit": "cell-updates/s",
+        "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_max / max(done, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if sc.real_bits == 32 else "f64", "data": "synthetic",
+        "coupled_steps_per_s": world * done / (ms_max * 1e-3),
+        "agent_updates_per_s": world * active * done / (ms_max * 1e-3),
+        "steps_executed": done,
+        "config": {"workload": f"config{args.config}: {sc.name}", "nx": sc.nx, "ny": sc.ny, "dx": sc.dx,
+                   "pedestrians": npeds, "active_pedestrians": active,
+                   "l2_policy": "inputs larger than L2 (no flush)" if ncell * fb > 126e6 else "working set fits L2: latency-bound config, roofline not meaningful",
+                   "flood_variant": args.flood_variant, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": world * ncell * e2e_done / e2e_s, "unit": "cell-updates/s",
+                "h2d_bytes_per_step": h2d / e2e_done, "d2h_bytes_per_step": d2h / e2e_done,
+                "steps": e2e_done, "seconds": e2e_s,
+                "what": "sim_write_flood+sim_write_peds from pinned host, sim_step, sim_read_conserved+sim_read_peds+sim_get_stats to host"},
+        "gpu_launches": int(done * kps),
+        "roofline": {"bound": "hbm", "kernel": "flood_tile_kernel<float>" if args.flood_variant else "flood_cell_kernel<float>",
+                     "achieved": flood_gbs, "peak": peak, "unit": "GB/s", "frac": flood_gbs / peak,
+                     "peak_source": peak_src, "frac_of_8TBs_spec": flood_gbs / 8000.0,
+                     "bytes_per_cell": fb, "kernel_ms": flood_ms, "traffic": None,
+                     "timed_with": f"cudaEvent before each launch over {KP} steps (sim_step_profiled) right after the timed region"},
+        "kernels_ms_per_step": {k: v / KP for k, v in kms.items()},
+        "ped_roofline": {"bound": "hbm", "kernels": "bin_count+bin_scan+scatter+ped_step", "achieved": ped_gbs, "peak": peak,
+                         "unit": "GB/s", "frac": ped_gbs / peak, "ms": ped_ms},
+        "cpu_baseline": cpu,
+        "final": {"t": st1["t"], "volume": st1["volume"], "max_h": st1["max_h"], "hist": st1["hist"],
+                  "neg_depth_clamps": st1["neg_depth_clamps"]},
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--flood-variant", type=int, default=1, choices=[0, 1])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,191 @@
+/*
+ * floodped.h -- C ABI of libfloodped.so: the coupled flood-pedestrian timestep of
+ * Shirvani, Kesserwani & Richmond, "Agent-based simulator of dynamic flood-people
+ * interactions" (arXiv 1908.05232), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations: "P:L<n>" = line n of the paper text; "C<nn>" = the reading of
+ * that number in DESIGN.md section 3 (where the paper is silent, ambiguous or garbled).
+ *
+ * One coupled step n -> n+1, every read at level n (the paper's simultaneous update of
+ * all agents):
+ *   (O) pedestrians per cell N_p -> roughness n = n0 (1 + min(N_p, n_cap))
+ *   (F) flood cells: first-order finite-volume update of U = [h, hu, hv], Eq. (2),
+ *       Riemann fluxes on hydrostatically reconstructed states, Manning friction
+ *   (T) t += dt ; dt for the next step from the CFL criterion, on the device
+ *   (B) pedestrians binned by counting sort + prefix scan (replaces FLAMEGPU's
+ *       per-cell messages)
+ *   (P) pedestrian step: HR = (V + 0.5) h -> Table 1 state and speed, navigation,
+ *       social force over adjacent bins, move, responder actions, exit
+ *   (S) sandbags dropped this step raise the bed z of the barrier line
+ *
+ * Conventions
+ *  - Every function returns SIM_OK (0) or a negative SIM_E* code; nothing throws or aborts
+ *    across this boundary.  sim_last_error() gives a human-readable reason.
+ *  - Grid arrays are row-major [j][i], ny rows of nx cells; cell (i,j) has centre
+ *    ((i+.5)dx, (j+.5)dy); a cell index is j*nx+i.
+ *  - "real" arrays hold float when grid.real_bits == 32 and double when it is 64; that is
+ *    also the precision the kernels compute in.
+ *  - INPUT pointers of sim_create / sim_write_* are HOST pointers, borrowed for the call and
+ *    copied.  OUTPUT pointers of sim_read_* may be HOST or DEVICE pointers (detected with
+ *    cudaPointerGetAttributes); the caller owns them and they must hold the stated length.
+ *  - If `workspace` is non-NULL it is a DEVICE buffer of at least sim_workspace_bytes()
+ *    bytes (e.g. a torch.empty uint8 tensor) that holds ALL device state; the library then
+ *    never calls cudaMalloc and the caller frees the buffer after sim_destroy.
+ *  - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  sim_step only enqueues
+ *    work on it and never synchronises; sim_read_*, sim_get_stats synchronise it.
+ *  - A handle is not thread-safe; distinct handles are independent.
+ *  - There is no CPU fallback: without a CUDA device sim_create fails with SIM_ECUDA.
+ */
+#ifndef FLOODPED_H
+#define FLOODPED_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SIM_OK          0
+#define SIM_EINVAL     -1   /* bad argument (which one: sim_last_error)          */
+#define SIM_ENOMEM     -2   /* workspace too small or device allocation failed   */
+#define SIM_ECUDA      -3   /* CUDA runtime error, or no device                  */
+#define SIM_ENOTFINITE -4   /* a non-finite depth or position was found at read  */
+
+/* cell sides for inflow faces */
+#define SIM_SIDE_W 0
+#define SIM_SIDE_E 1
+#define SIM_SIDE_S 2
+#define SIM_SIDE_N 3
+/* flood-risk state of a pedestrian: Table 1 plus "dry" (C17) */
+#define SIM_STATE_DRY 0
+#define SIM_STATE_LOW 1
+#define SIM_STATE_MEDIUM 2
+#define SIM_STATE_HIGH 3
+#define SIM_STATE_HIGHEST 4
+/* responder finite-state machine; evacuees are always SIM_FSM_EVACUATE */
+#define SIM_FSM_EVACUATE 0
+#define SIM_FSM_TO_STORAGE 1
+#define SIM_FSM_PICKING 2
+#define SIM_FSM_TO_BARRIER 3
+#define SIM_FSM_DROPPING 4
+/* navigation direction codes: 0..7 = E,NE,N,NW,W,SW,S,SE */
+#define SIM_DIR_NONE 255
+
+typedef struct sim sim_t;                       /* opaque, owned by the library */
+
+typedef struct {
+    int32_t nx, ny;
+    double  dx, dy;                             /* cell size, m                  */
+    int32_t real_bits;                          /* 32 or 64                               */
+} sim_grid_t;
+
+typedef struct {                                /* flood agents' initial state    */
+    const void    *z;                           /* [ny*nx] real, bed elevation            */
+    const uint8_t *mask;                        /* [ny*nx] 1 = solid/impassable; NULL = none (C16) */
+    const void    *h0, *u0, *v0;                /* [ny*nx] real; NULL = 0                 */
+} sim_topo_t;
+
+typedef struct {                                /* pedestrian agents        */
+    int32_t        n;
+    const void    *x, *y, *vx, *vy, *v_pref;    /* [n] real; v_pref = dry walking speed */
+    const uint8_t *role;                        /* [n] 0 evacuee, 1 responder             */
+} sim_peds_t;
+
+typedef struct {
+    /* hydrodynamics */
+    double  g, cfl, dt_max, h_dry;              /* 9.81, 0.5, <=0 => C10 default, 1e-3 (C5, C7, C9) */
+    int32_t couple_roughness, n_cap;            /* people -> roughness on/off; cap 20; n_cap <= 255 */
+    /* inflow (C14): faces on the domain edge, wall for momentum, mass flux Q(t)/length */
+    int32_t        n_inflow_faces;
+    const int32_t *inflow_cell;                 /* [n_inflow_faces] cell index on the edge named by side */
+    const uint8_t *inflow_side;                 /* [n_inflow_faces] SIM_SIDE_*            */
+    int32_t        n_hydro;
+    const double  *hydro_t, *hydro_q;           /* [n_hydro] piecewise-linear Q(t), m3/s, t increasing */
+    /* Table 1 */
+    double  hr_edges[4];                        /* 0.75 1.5 2.5 20 (4th unused, C17)      */
+    double  speed_wet[4];                       /* 1.8 0.9 0.45 0.0 m/s                   */
+    /* social force (C24-C26) */
+    double  tau, A_s, B_s, radius, R_int, vmax_factor;   /* .5 25 .08 .3 1.0 1.3          */
+    /* navigation (C28) */
+    int32_t        n_targets;
+    const uint8_t *nav_dir;                     /* [n_targets][ny*nx] direction code      */
+    int32_t        exit_target, storage_target, drop_target;
+    int32_t        n_exit_cells;
+    const int32_t *exit_cells;                  /* [n_exit_cells], at most 16             */
+    int32_t        storage_cell, drop_cell, arrive_cells;   /* arrival = Chebyshev cell distance <= arrive_cells (C29, C31) */
+    /* sandbag barrier (C31-C36) */
+    int32_t        n_line;
+    const int32_t *line_cells;                  /* [n_line] barrier cells in filling order, not solid */
+    int32_t        bags_per_cell_layer, n_layers;
+    double  layer_thickness, t_pick, t_drop;    /* 0.25 m, 30 s, 30 s                     */
+    double  t_end;                              /* steps are no-ops once t >= t_end; INFINITY = off */
+} sim_params_t;
+
+typedef struct {
+    double  t, dt;                              /* time reached; dt of the NEXT step      */
+    int64_t step;
+    double  volume, max_h, max_hr;              /* volume summed in fp64                  */
+    int64_t hist[6];                            /* dry low medium high highest exited     */
+    int64_t neg_depth_clamps;                   /* C12                                    */
+    double  clamped_volume;
+    int32_t cursor, layer, bags, barrier_complete;
+    int64_t deposits;
+} sim_stats_t;
+
+/* Bytes of device workspace sim_create needs for this problem. */
+int sim_workspace_bytes(const sim_grid_t *grid, int32_t n_peds, const sim_params_t *params,
+                        size_t *bytes);
+
+/* Validate, place all state in device memory, upload, compute the first dt. */
+int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const void *manning /* [ny*nx] real */,
+               const sim_peds_t *peds, const sim_params_t *params,
+               void *workspace /* device or NULL */, void *cuda_stream, sim_t **out);
+
+/* Enqueue n coupled steps on the stream; asynchronous; dt and t stay on the device. */
+int sim_step(sim_t *s, int64_t n);
+
+/* The same n steps launched kernel by kernel (no graph) with a CUDA event before each launch;
+ * synchronises.  kernel_ms[8] receives the summed device time in ms of: 0 bin count, 1 bin scan,
+ * 2 scatter, 3 pedestrian step, 4 flood step, 5 tail; 6, 7 unused.  For measurement. */
+int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms);
+
+/* Flood agents' recorded fields: depth, velocities (0 where h <= h_dry, C8), bed,
+ * hazard rate.  Each [ny*nx] real; any pointer may be NULL. */
+int sim_read_flood(sim_t *s, void *h, void *u, void *v, void *z, void *hr);
+/* The conserved state [h, hu, hv] itself. */
+int sim_read_conserved(sim_t *s, void *h, void *qx, void *qy);
+/* N_p per cell as used by the most recent step (saturated at 255). [ny*nx] */
+int sim_read_occupancy(sim_t *s, uint8_t *np_cell);
+/* Pedestrians in ORIGINAL index order, length n: position, velocity (real), risk
+ * state, FSM, active flag (0 = has left), containing cell, wait timer (real). Any may be NULL. */
+int sim_read_peds(sim_t *s, void *x, void *y, void *vx, void *vy, uint8_t *state, uint8_t *fsm,
+                  uint8_t *active, int32_t *cell, void *timer);
+int sim_get_stats(sim_t *s, sim_stats_t *out);
+
+/* ---- test hooks ---- */
+/* Bin the pedestrians of the current level without stepping: key[n] in original order (bin
+ * index, n_bins for inactive), order[n] = original index held by each sorted slot,
+ * start[n_bins+2] exclusive scan (start[n_bins+1] = n).  Bins are k x k cells,
+ * k = ceil(R_int / min(dx,dy)) (C26).  Pointers may be NULL; HOST or DEVICE. */
+int sim_bin_peds(sim_t *s, int32_t *key, int32_t *order, int32_t *start,
+                 int32_t *n_bins_x, int32_t *n_bins_y, int32_t *k);
+/* Re-inject state (HOST pointers, NULL = keep). */
+int sim_write_flood(sim_t *s, const void *h, const void *qx, const void *qy, const void *z);
+int sim_write_peds(sim_t *s, const void *x, const void *y, const void *vx, const void *vy,
+                   const uint8_t *fsm, const uint8_t *active, const void *timer);
+int sim_set_time(sim_t *s, double t, double dt);
+int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete);
+/* Choose the flood kernel: 0 = reference-shaped (one thread per cell, 4 faces each),
+ * 1 = tiled (each face once, shared-memory staging).  Default 1. */
+int sim_set_flood_variant(sim_t *s, int32_t variant);
+/* Number of kernels sim_step launches per coupled step (for launch accounting). */
+int sim_kernels_per_step(const sim_t *s);
+
+const char *sim_last_error(const sim_t *s);     /* s may be NULL: error of the last failed create */
+void sim_destroy(sim_t *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

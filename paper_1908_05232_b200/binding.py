@@ -1,0 +1,314 @@
+"""Thin ctypes binding over the C ABI of libfloodped.so (include/floodped.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels.  PyTorch supplies
+the device workspace (`torch.empty`) and the stream; there is no CPU fallback -- if the library
+or a CUDA device is missing, construction raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfloodped.so")
+
+SIM_OK, SIM_EINVAL, SIM_ENOMEM, SIM_ECUDA, SIM_ENOTFINITE = 0, -1, -2, -3, -4
+
+EXPORTS = [
+    "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
+    "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
+    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_set_flood_variant",
+    "sim_kernels_per_step", "sim_last_error", "sim_destroy",
+]
+
+_vp = C.c_void_p
+_u8p = C.POINTER(C.c_uint8)
+_i32p = C.POINTER(C.c_int32)
+_f64p = C.POINTER(C.c_double)
+
+
+class SimGrid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dx", C.c_double), ("dy", C.c_double),
+                ("real_bits", C.c_int32)]
+
+
+class SimTopo(C.Structure):
+    _fields_ = [("z", _vp), ("mask", _u8p), ("h0", _vp), ("u0", _vp), ("v0", _vp)]
+
+
+class SimPeds(C.Structure):
+    _fields_ = [("n", C.c_int32), ("x", _vp), ("y", _vp), ("vx", _vp), ("vy", _vp), ("v_pref", _vp),
+                ("role", _u8p)]
+
+
+class SimParams(C.Structure):
+    _fields_ = [
+        ("g", C.c_double), ("cfl", C.c_double), ("dt_max", C.c_double), ("h_dry", C.c_double),
+        ("couple_roughness", C.c_int32), ("n_cap", C.c_int32),
+        ("n_inflow_faces", C.c_int32), ("inflow_cell", _i32p), ("inflow_side", _u8p),
+        ("n_hydro", C.c_int32), ("hydro_t", _f64p), ("hydro_q", _f64p),
+        ("hr_edges", C.c_double * 4), ("speed_wet", C.c_double * 4),
+        ("tau", C.c_double), ("A_s", C.c_double), ("B_s", C.c_double), ("radius", C.c_double),
+        ("R_int", C.c_double), ("vmax_factor", C.c_double),
+        ("n_targets", C.c_int32), ("nav_dir", _u8p),
+        ("exit_target", C.c_int32), ("storage_target", C.c_int32), ("drop_target", C.c_int32),
+        ("n_exit_cells", C.c_int32), ("exit_cells", _i32p),
+        ("storage_cell", C.c_int32), ("drop_cell", C.c_int32), ("arrive_cells", C.c_int32),
+        ("n_line", C.c_int32), ("line_cells", _i32p),
+        ("bags_per_cell_layer", C.c_int32), ("n_layers", C.c_int32),
+        ("layer_thickness", C.c_double), ("t_pick", C.c_double), ("t_drop", C.c_double),
+        ("t_end", C.c_double),
+    ]
+
+
+class SimStats(C.Structure):
+    _fields_ = [
+        ("t", C.c_double), ("dt", C.c_double), ("step", C.c_int64),
+        ("volume", C.c_double), ("max_h", C.c_double), ("max_hr", C.c_double),
+        ("hist", C.c_int64 * 6), ("neg_depth_clamps", C.c_int64), ("clamped_volume", C.c_double),
+        ("cursor", C.c_int32), ("layer", C.c_int32), ("bags", C.c_int32), ("barrier_complete", C.c_int32),
+        ("deposits", C.c_int64),
+    ]
+
+
+class FloodpedError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libfloodped error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """dlopen libfloodped.so and declare the prototypes.  Raises if the library is missing:
+    there is no fallback path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            f"{path} is missing: build it with `python -m paper_1908_05232_b200.build` "
+            "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    L.sim_workspace_bytes.argtypes = [C.POINTER(SimGrid), C.c_int32, C.POINTER(SimParams), C.POINTER(C.c_size_t)]
+    L.sim_create.argtypes = [C.POINTER(SimGrid), C.POINTER(SimTopo), _vp, C.POINTER(SimPeds),
+                             C.POINTER(SimParams), _vp, _vp, C.POINTER(_vp)]
+    L.sim_step.argtypes = [_vp, C.c_int64]
+    L.sim_step_profiled.argtypes = [_vp, C.c_int64, _f64p]
+    L.sim_read_flood.argtypes = [_vp] * 6
+    L.sim_read_conserved.argtypes = [_vp] * 4
+    L.sim_read_occupancy.argtypes = [_vp, _vp]
+    L.sim_read_peds.argtypes = [_vp] * 10
+    L.sim_get_stats.argtypes = [_vp, C.POINTER(SimStats)]
+    L.sim_bin_peds.argtypes = [_vp, _vp, _vp, _vp, _i32p, _i32p, _i32p]
+    L.sim_write_flood.argtypes = [_vp] * 5
+    L.sim_write_peds.argtypes = [_vp] * 8
+    L.sim_set_time.argtypes = [_vp, C.c_double, C.c_double]
+    L.sim_set_barrier.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32]
+    L.sim_set_flood_variant.argtypes = [_vp, C.c_int32]
+    L.sim_kernels_per_step.argtypes = [_vp]
+    L.sim_last_error.argtypes = [_vp]
+    L.sim_last_error.restype = C.c_char_p
+    L.sim_destroy.argtypes = [_vp]
+    L.sim_destroy.restype = None
+    for name in EXPORTS:
+        if name not in ("sim_last_error", "sim_destroy"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _np_ptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+class _Marshalled:
+    """Host-side C structs for a Scenario; keeps the numpy arrays alive."""
+
+    def __init__(self, sc):
+        real = np.float64 if sc.real_bits == 64 else np.float32
+        self.real = real
+        self.keep = []
+
+        def arr(a, dtype):
+            if a is None:
+                return None
+            a = np.ascontiguousarray(a, dtype=dtype)
+            self.keep.append(a)
+            return a
+
+        def typed(a, dtype, ptype):
+            a = arr(a, dtype)
+            return C.cast(None, ptype) if a is None or a.size == 0 else a.ctypes.data_as(ptype)
+
+        self.grid = SimGrid(sc.nx, sc.ny, sc.dx, sc.dy, sc.real_bits)
+        self.topo = SimTopo(_np_ptr(arr(sc.z, real)), typed(sc.mask, np.uint8, _u8p),
+                            _np_ptr(arr(sc.h0, real)), _np_ptr(arr(sc.u0, real)), _np_ptr(arr(sc.v0, real)))
+        self.manning = arr(sc.manning, real)
+        n = int(sc.px.shape[0])
+        self.peds = SimPeds(n, _np_ptr(arr(sc.px, real)), _np_ptr(arr(sc.py, real)),
+                            _np_ptr(arr(sc.pvx, real)), _np_ptr(arr(sc.pvy, real)),
+                            _np_ptr(arr(sc.pvpref, real)), typed(sc.prole, np.uint8, _u8p))
+        p = SimParams()
+        p.g, p.cfl, p.dt_max, p.h_dry = sc.g, sc.cfl, sc.dt_max, sc.h_dry
+        p.couple_roughness, p.n_cap = sc.couple_roughness, sc.n_cap
+        p.n_inflow_faces = len(sc.inflow_cell)
+        p.inflow_cell = typed(sc.inflow_cell, np.int32, _i32p)
+        p.inflow_side = typed(sc.inflow_side, np.uint8, _u8p)
+        p.n_hydro = len(sc.hydro_t)
+        p.hydro_t = typed(sc.hydro_t, np.float64, _f64p)
+        p.hydro_q = typed(sc.hydro_q, np.float64, _f64p)
+        p.hr_edges = (C.c_double * 4)(*sc.hr_edges)
+        p.speed_wet = (C.c_double * 4)(*sc.speed_wet)
+        p.tau, p.A_s, p.B_s, p.radius, p.R_int, p.vmax_factor = sc.tau, sc.A_s, sc.B_s, sc.radius, sc.R_int, sc.vmax_factor
+        nav = np.ascontiguousarray(sc.nav_dir, dtype=np.uint8).reshape(-1, sc.nx * sc.ny)
+        p.n_targets = nav.shape[0]
+        p.nav_dir = typed(nav, np.uint8, _u8p)
+        p.exit_target, p.storage_target, p.drop_target = sc.exit_target, sc.storage_target, sc.drop_target
+        p.n_exit_cells = len(sc.exit_cells)
+        p.exit_cells = typed(sc.exit_cells, np.int32, _i32p)
+        p.storage_cell, p.drop_cell, p.arrive_cells = sc.storage_cell, sc.drop_cell, sc.arrive_cells
+        p.n_line = len(sc.line_cells)
+        p.line_cells = typed(sc.line_cells, np.int32, _i32p)
+        p.bags_per_cell_layer, p.n_layers = sc.bags_per_cell_layer, sc.n_layers
+        p.layer_thickness, p.t_pick, p.t_drop, p.t_end = sc.layer_thickness, sc.t_pick, sc.t_drop, sc.t_end
+        self.params = p
+
+
+def workspace_bytes(sc) -> int:
+    L = load_library()
+    m = _Marshalled(sc)
+    out = C.c_size_t()
+    rc = L.sim_workspace_bytes(C.byref(m.grid), m.peds.n, C.byref(m.params), C.byref(out))
+    if rc != SIM_OK:
+        raise FloodpedError(rc, L.sim_last_error(None).decode())
+    return out.value
+
+
+class Sim:
+    """One simulation handle on the current CUDA device / current torch stream."""
+
+    def __init__(self, sc, device="cuda:0", use_torch_workspace=True, stream=None):
+        import torch
+
+        L = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: libfloodped has no CPU fallback")
+        self._L = L
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.real = np.float64 if sc.real_bits == 64 else np.float32
+        self.nx, self.ny, self.ncell, self.n_peds = sc.nx, sc.ny, sc.nx * sc.ny, int(sc.px.shape[0])
+        m = _Marshalled(sc)
+        self._ws = None
+        ws_ptr = None
+        if use_torch_workspace:
+            nbytes = C.c_size_t()
+            rc = L.sim_workspace_bytes(C.byref(m.grid), m.peds.n, C.byref(m.params), C.byref(nbytes))
+            if rc != SIM_OK:
+                raise FloodpedError(rc, L.sim_last_error(None).decode())
+            self._ws = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+            ws_ptr = C.c_void_p(self._ws.data_ptr())
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        rc = L.sim_create(C.byref(m.grid), C.byref(m.topo), _np_ptr(m.manning), C.byref(m.peds),
+                          C.byref(m.params), ws_ptr, C.c_void_p(self._stream.cuda_stream), C.byref(h))
+        if rc != SIM_OK:
+            raise FloodpedError(rc, L.sim_last_error(None).decode())
+        self._h = h
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.sim_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    __del__ = close
+
+    def _chk(self, rc):
+        if rc != SIM_OK:
+            raise FloodpedError(rc, self._L.sim_last_error(self._h).decode())
+
+    # -- the path
+    def step(self, n=1):
+        self._chk(self._L.sim_step(self._h, int(n)))
+
+    KERNELS = ("bin_count", "bin_scan", "scatter", "ped_step", "flood_step", "tail")
+
+    def step_profiled(self, n=1) -> dict:
+        """n steps with per-kernel CUDA-event timing; returns summed ms per kernel."""
+        ms = (C.c_double * 8)()
+        self._chk(self._L.sim_step_profiled(self._h, int(n), ms))
+        return {k: ms[i] for i, k in enumerate(self.KERNELS)}
+
+    def kernels_per_step(self) -> int:
+        return self._L.sim_kernels_per_step(self._h)
+
+    def set_flood_variant(self, v):
+        self._chk(self._L.sim_set_flood_variant(self._h, int(v)))
+
+    # -- read-back (host numpy)
+    def read_flood(self, fields=("h", "u", "v", "z", "hr")):
+        out = {k: np.empty(self.ncell, self.real) for k in fields}
+        self._chk(self._L.sim_read_flood(self._h, *[_np_ptr(out.get(k)) for k in ("h", "u", "v", "z", "hr")]))
+        return out
+
+    def read_conserved(self):
+        out = {k: np.empty(self.ncell, self.real) for k in ("h", "qx", "qy")}
+        self._chk(self._L.sim_read_conserved(self._h, *[_np_ptr(out[k]) for k in ("h", "qx", "qy")]))
+        return out
+
+    def read_conserved_into(self, h_ptr, qx_ptr, qy_ptr):
+        """Raw pointers (host or device), e.g. pinned torch tensors' data_ptr()."""
+        self._chk(self._L.sim_read_conserved(self._h, C.c_void_p(h_ptr), C.c_void_p(qx_ptr), C.c_void_p(qy_ptr)))
+
+    def read_occupancy(self):
+        a = np.empty(self.ncell, np.uint8)
+        self._chk(self._L.sim_read_occupancy(self._h, _np_ptr(a)))
+        return a
+
+    def read_peds(self):
+        n = self.n_peds
+        out = {k: np.empty(n, self.real) for k in ("x", "y", "vx", "vy", "timer")}
+        out.update({k: np.empty(n, np.uint8) for k in ("state", "fsm", "active")})
+        out["cell"] = np.empty(n, np.int32)
+        self._chk(self._L.sim_read_peds(self._h, *[_np_ptr(out[k]) for k in
+                                                    ("x", "y", "vx", "vy", "state", "fsm", "active", "cell", "timer")]))
+        return out
+
+    def stats(self) -> dict:
+        st = SimStats()
+        self._chk(self._L.sim_get_stats(self._h, C.byref(st)))
+        d = {k: getattr(st, k) for k, _ in SimStats._fields_ if k != "hist"}
+        d["hist"] = list(st.hist)
+        return d
+
+    # -- test hooks
+    def bin_peds(self):
+        nbx, nby, k = C.c_int32(), C.c_int32(), C.c_int32()
+        self._chk(self._L.sim_bin_peds(self._h, None, None, None, C.byref(nbx), C.byref(nby), C.byref(k)))
+        nb = nbx.value * nby.value
+        key = np.empty(self.n_peds, np.int32); order = np.empty(self.n_peds, np.int32)
+        start = np.empty(nb + 2, np.int32)
+        self._chk(self._L.sim_bin_peds(self._h, _np_ptr(key), _np_ptr(order), _np_ptr(start), None, None, None))
+        return {"key": key, "order": order, "start": start, "nbx": nbx.value, "nby": nby.value, "k": k.value}
+
+    def write_flood(self, h=None, qx=None, qy=None, z=None):
+        a = [None if v is None else np.ascontiguousarray(v, self.real) for v in (h, qx, qy, z)]
+        self._chk(self._L.sim_write_flood(self._h, *[_np_ptr(v) for v in a]))
+
+    def write_peds(self, x=None, y=None, vx=None, vy=None, fsm=None, active=None, timer=None):
+        f = [None if v is None else np.ascontiguousarray(v, self.real) for v in (x, y, vx, vy)]
+        b = [None if v is None else np.ascontiguousarray(v, np.uint8) for v in (fsm, active)]
+        t = None if timer is None else np.ascontiguousarray(timer, self.real)
+        self._chk(self._L.sim_write_peds(self._h, *[_np_ptr(v) for v in f], *[_np_ptr(v) for v in b], _np_ptr(t)))
+
+    def set_time(self, t, dt):
+        self._chk(self._L.sim_set_time(self._h, float(t), float(dt)))
+
+    def set_barrier(self, cursor, layer, bags, complete):
+        self._chk(self._L.sim_set_barrier(self._h, int(cursor), int(layer), int(bags), int(complete)))

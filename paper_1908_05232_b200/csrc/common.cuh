@@ -1,0 +1,67 @@
+// common.cuh -- device-side control block and small helpers shared by the kernels of
+// libfloodped.so.  (Nothing here is shared with oracle/: the oracle is a separate C program.)
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+namespace fp {
+
+// Everything that changes from step to step and must not round-trip through the host
+// (the CFL time step is global and adaptive; north_star: "no host round-trip").
+// One instance lives in device memory; kernels of a step read it, the tail kernel advances it.
+struct Ctl {
+    double t, dt;                    // time reached; dt of the step being taken
+    double t_end, dt_max, cfl;
+    double q_in;                     // inflow per unit width for the step being taken, m2/s
+    double clamped_volume;           // C12 accounting
+    unsigned long long lam_bits;     // bits of max over wet cells of (|u|+c)/dx, (|v|+c)/dy at n+1
+    unsigned long long neg_clamps;
+    long long step, deposits;
+    int parity;                      // which of the two flood buffers holds level n
+    int halt;                        // t >= t_end: every kernel of the step returns at once
+    int D;                           // sandbag deposits of the step being taken
+    int cursor, layer, bags, complete;
+    unsigned int scan_epoch;         // makes the look-back flags of the scan self-resetting
+    unsigned int scan_ticket;        // dynamic tile index of the scan
+};
+
+template <typename T> struct Vec4 { T v[4]; };
+template <> struct __align__(16) Vec4<float> { float v[4]; };
+template <> struct __align__(32) Vec4<double> { double v[4]; };
+
+template <typename T> __device__ __forceinline__ T solid_z();
+template <> __device__ __forceinline__ float solid_z<float>() { return CUDART_INF_F; }
+template <> __device__ __forceinline__ double solid_z<double>() { return CUDART_INF; }
+
+__device__ __forceinline__ bool is_solid(float z) { return z == CUDART_INF_F; }
+__device__ __forceinline__ bool is_solid(double z) { return z == CUDART_INF; }
+
+// correctly rounded single operations (never contracted into FMA): the integer-valued
+// decisions of the pedestrian step are taken with these so that they are reproducible
+// bit for bit by a float replay on the CPU
+__device__ __forceinline__ float  mul_rn(float a, float b)   { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float  add_rn(float a, float b)   { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float  div_rn(float a, float b)   { return __fdiv_rn(a, b); }
+__device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
+
+__device__ __forceinline__ float  fast_rcp(float a)  { return __frcp_rn(a); }
+__device__ __forceinline__ double fast_rcp(double a) { return 1.0 / a; }
+__device__ __forceinline__ float  real_sqrt(float a)  { return sqrtf(a); }
+__device__ __forceinline__ double real_sqrt(double a) { return sqrt(a); }
+__device__ __forceinline__ float  real_exp(float a)  { return __expf(a); }
+__device__ __forceinline__ double real_exp(double a) { return exp(a); }
+// h^(7/3) for the Manning term
+__device__ __forceinline__ float  pow73(float h)  { return h * h * cbrtf(h); }
+__device__ __forceinline__ double pow73(double h) { return h * h * cbrt(h); }
+
+__device__ __forceinline__ void atomic_max_lambda(Ctl *ctl, double lam)
+{
+    // lam >= 0: the IEEE bit pattern of non-negative doubles is ordered like the integers
+    atomicMax(&ctl->lam_bits, (unsigned long long)__double_as_longlong(lam));
+}
+
+}  // namespace fp

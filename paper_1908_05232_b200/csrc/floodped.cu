@@ -1,0 +1,817 @@
+// floodped.cu -- the C ABI of include/floodped.h over the kernels in flood.cuh / peds.cuh.
+// Host code only marshals, validates, places state in one device workspace and enqueues
+// kernels (as CUDA graphs); every step of the path runs in the kernels.
+#include "../../include/floodped.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "flood.cuh"
+#include "peds.cuh"
+
+using namespace fp;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr int GRAPH_CHUNK = 32;     // coupled steps per large graph launch
+
+struct Bump {                       // carve device state out of one workspace
+    char *base = nullptr; size_t off = 0, cap = 0; bool dry = true;
+    template <typename U> U *take(size_t n)
+    {
+        off = (off + 255) & ~size_t(255);
+        U *p = dry ? nullptr : reinterpret_cast<U *>(base + off);
+        off += n * sizeof(U);
+        return p;
+    }
+};
+
+}  // namespace
+
+struct sim {
+    sim_grid_t grid{};
+    sim_params_t prm{};             // scalar copy; pointers inside are NOT valid after create
+    int ncell = 0, np = 0, kbin = 1, nbx = 0, nby = 0, nbins = 0;
+    int n_inflow = 0, n_hydro = 0, n_line = 0, n_targets = 0;
+    double inflow_length = 0.0;
+    cudaStream_t stream = nullptr, cap_stream = nullptr;
+    void *ws = nullptr; size_t ws_bytes = 0; bool own_ws = false;
+    // device arrays (void*: real type decided by grid.real_bits)
+    void *h[2]{}, *qx[2]{}, *qy[2]{}, *zs = nullptr, *z0 = nullptr, *n0 = nullptr, *scratch_real[3]{};
+    uint8_t *occ = nullptr, *mask = nullptr, *inflow[4]{}, *nav = nullptr;
+    int32_t *line_cells = nullptr;
+    double *hydro_t = nullptr, *hydro_q = nullptr;
+    struct { void *x, *y, *vx, *vy, *vpref, *timer; uint8_t *role, *fsm, *state, *active; int32_t *id, *cell; } P[2]{};
+    void *ped_out[5]{};             // gather targets (x y vx vy timer) in original order
+    uint8_t *ped_out_u8[3]{};
+    int32_t *ped_out_i32[2]{};
+    int32_t *key = nullptr, *off = nullptr, *count = nullptr, *start = nullptr, *cellprev = nullptr;
+    unsigned long long *scan_status = nullptr;
+    Ctl *ctl = nullptr;
+    double *stat_d = nullptr;       // [4] volume, max_h, max_hr, n_bad ; [4] ped bad
+    unsigned long long *stat_hist = nullptr;   // [6]
+    int flood_variant = 1;
+    int exit_i[16]{}, exit_j[16]{};
+    cudaGraphExec_t graph1 = nullptr, graphN = nullptr;
+    std::string err;
+};
+
+namespace {
+
+int fail(sim *s, int code, const std::string &msg)
+{
+    if (s) s->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(s, SIM_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));         \
+    } while (0)
+
+size_t real_size(const sim *s) { return s->grid.real_bits == 64 ? 8 : 4; }
+
+// Lay out (dry = true: only measure) all device state.
+size_t layout(sim *s, Bump &b)
+{
+    const size_t rs = real_size(s), nc = (size_t)s->ncell, np = (size_t)s->np;
+    auto real = [&](size_t n) { return (void *)b.take<char>(n * rs); };
+    s->ctl = b.take<Ctl>(1);
+    s->stat_d = b.take<double>(8);
+    s->stat_hist = b.take<unsigned long long>(8);
+    for (int k = 0; k < 2; ++k) { s->h[k] = real(nc); s->qx[k] = real(nc); s->qy[k] = real(nc); }
+    s->zs = real(nc); s->z0 = real(nc); s->n0 = real(nc);
+    for (int k = 0; k < 3; ++k) s->scratch_real[k] = real(nc);
+    s->occ = b.take<uint8_t>(nc); s->mask = b.take<uint8_t>(nc);
+    s->inflow[0] = b.take<uint8_t>(s->grid.ny); s->inflow[1] = b.take<uint8_t>(s->grid.ny);
+    s->inflow[2] = b.take<uint8_t>(s->grid.nx); s->inflow[3] = b.take<uint8_t>(s->grid.nx);
+    s->nav = b.take<uint8_t>((size_t)s->n_targets * nc);
+    s->line_cells = b.take<int32_t>(s->n_line + 1);
+    s->hydro_t = b.take<double>(s->n_hydro + 1); s->hydro_q = b.take<double>(s->n_hydro + 1);
+    for (int k = 0; k < 2; ++k) {
+        s->P[k].x = real(np); s->P[k].y = real(np); s->P[k].vx = real(np); s->P[k].vy = real(np);
+        s->P[k].vpref = real(np); s->P[k].timer = real(np);
+        s->P[k].role = b.take<uint8_t>(np); s->P[k].fsm = b.take<uint8_t>(np);
+        s->P[k].state = b.take<uint8_t>(np); s->P[k].active = b.take<uint8_t>(np);
+        s->P[k].id = b.take<int32_t>(np); s->P[k].cell = b.take<int32_t>(np);
+    }
+    for (int k = 0; k < 5; ++k) s->ped_out[k] = real(np);
+    for (int k = 0; k < 3; ++k) s->ped_out_u8[k] = b.take<uint8_t>(np);
+    for (int k = 0; k < 2; ++k) s->ped_out_i32[k] = b.take<int32_t>(np);
+    s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(np);
+    s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
+    s->scan_status = b.take<unsigned long long>((size_t)(s->nbins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1);
+    return (b.off + 255) & ~size_t(255);
+}
+
+int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t *p)
+{
+    if (!g || !p) return fail(s, SIM_EINVAL, "null grid or params");
+    if (g->nx <= 0 || g->ny <= 0 || (long long)g->nx * g->ny > 0x7fffffffLL)
+        return fail(s, SIM_EINVAL, "nx, ny must be positive and nx*ny < 2^31");
+    if (!(g->dx > 0) || !(g->dy > 0)) return fail(s, SIM_EINVAL, "dx, dy must be positive");
+    if (g->real_bits != 32 && g->real_bits != 64) return fail(s, SIM_EINVAL, "real_bits must be 32 or 64");
+    if (n_peds < 0) return fail(s, SIM_EINVAL, "negative pedestrian count");
+    if (!(p->R_int > 0)) return fail(s, SIM_EINVAL, "R_int must be positive");
+    if (p->n_targets < 1 || p->n_inflow_faces < 0 || p->n_hydro < 0 || p->n_line < 0 || p->n_exit_cells < 0)
+        return fail(s, SIM_EINVAL, "bad list length in params");
+    s->grid = *g;
+    s->ncell = g->nx * g->ny; s->np = n_peds;
+    const double dmin = g->dx < g->dy ? g->dx : g->dy;
+    s->kbin = (int)std::ceil(p->R_int / dmin); if (s->kbin < 1) s->kbin = 1;     // C26
+    s->nbx = (g->nx + s->kbin - 1) / s->kbin; s->nby = (g->ny + s->kbin - 1) / s->kbin;
+    s->nbins = s->nbx * s->nby;
+    s->n_inflow = p->n_inflow_faces; s->n_hydro = p->n_hydro; s->n_line = p->n_line; s->n_targets = p->n_targets;
+    return SIM_OK;
+}
+
+template <typename T> FloodArgs<T> flood_args(const sim *s)
+{
+    FloodArgs<T> a{};
+    a.nx = s->grid.nx; a.ny = s->grid.ny;
+    a.g = (T)s->prm.g; a.inv_dx = (T)(1.0 / s->grid.dx); a.inv_dy = (T)(1.0 / s->grid.dy);
+    a.h_dry = (T)s->prm.h_dry; a.cell_area = (T)(s->grid.dx * s->grid.dy);
+    a.couple = s->prm.couple_roughness; a.n_cap = s->prm.n_cap;
+    for (int k = 0; k < 2; ++k) { a.h[k] = (T *)s->h[k]; a.qx[k] = (T *)s->qx[k]; a.qy[k] = (T *)s->qy[k]; }
+    a.zs = (const T *)s->zs; a.n0 = (const T *)s->n0; a.occ = s->occ;
+    for (int k = 0; k < 4; ++k) a.inflow[k] = s->inflow[k];
+    a.ctl = s->ctl;
+    return a;
+}
+
+template <typename T> PedSoA<T> ped_soa(const sim *s, int k)
+{
+    PedSoA<T> p{};
+    p.x = (T *)s->P[k].x; p.y = (T *)s->P[k].y; p.vx = (T *)s->P[k].vx; p.vy = (T *)s->P[k].vy;
+    p.vpref = (T *)s->P[k].vpref; p.timer = (T *)s->P[k].timer;
+    p.role = s->P[k].role; p.fsm = s->P[k].fsm; p.state = s->P[k].state; p.active = s->P[k].active;
+    p.id = s->P[k].id; p.cell = s->P[k].cell;
+    return p;
+}
+
+template <typename T> PedArgs<T> ped_args(const sim *s)
+{
+    PedArgs<T> a{};
+    const sim_params_t &p = s->prm;
+    a.n = s->np; a.nx = s->grid.nx; a.ny = s->grid.ny;
+    a.kbin = s->kbin; a.nbx = s->nbx; a.nby = s->nby; a.nbins = s->nbins;
+    a.inv_dx = (T)(1.0 / s->grid.dx); a.inv_dy = (T)(1.0 / s->grid.dy);
+    a.h_dry = (T)p.h_dry;
+    for (int k = 0; k < 3; ++k) a.hr_edge[k] = (T)p.hr_edges[k];
+    for (int k = 0; k < 4; ++k) a.speed_wet[k] = (T)p.speed_wet[k];
+    a.inv_tau = (T)(1.0 / p.tau); a.A_s = (T)p.A_s; a.inv_B = (T)(1.0 / p.B_s); a.two_r = (T)(2.0 * p.radius);
+    a.R_int = (T)p.R_int; a.vmax_factor = (T)p.vmax_factor; a.t_pick = (T)p.t_pick; a.t_drop = (T)p.t_drop;
+    a.n_targets = p.n_targets; a.exit_target = p.exit_target; a.storage_target = p.storage_target;
+    a.drop_target = p.drop_target;
+    a.storage_i = p.storage_cell % s->grid.nx; a.storage_j = p.storage_cell / s->grid.nx;
+    a.drop_i = p.drop_cell % s->grid.nx; a.drop_j = p.drop_cell / s->grid.nx;
+    a.arrive = p.arrive_cells;
+    a.A = ped_soa<T>(s, 0); a.B = ped_soa<T>(s, 1);
+    a.key = s->key; a.off = s->off; a.count = s->count; a.start = s->start; a.cellprev = s->cellprev;
+    a.occ = s->occ; a.mask = s->mask; a.nav = s->nav;
+    for (int k = 0; k < 2; ++k) { a.h[k] = (const T *)s->h[k]; a.qx[k] = (const T *)s->qx[k]; a.qy[k] = (const T *)s->qy[k]; }
+    a.ctl = s->ctl;
+    return a;
+}
+
+template <typename T> TailArgs<T> tail_args(const sim *s)
+{
+    TailArgs<T> a{};
+    a.ctl = s->ctl; a.zs = (T *)s->zs; a.line_cells = s->line_cells;
+    a.n_line = s->n_line; a.bags_per_cell_layer = s->prm.bags_per_cell_layer; a.n_layers = s->prm.n_layers;
+    a.layer_thickness = (T)s->prm.layer_thickness;
+    a.hydro_t = s->hydro_t; a.hydro_q = s->hydro_q; a.n_hydro = s->n_hydro;
+    a.inv_inflow_length = s->inflow_length > 0 ? 1.0 / s->inflow_length : 0.0;
+    return a;
+}
+
+// ---- enqueue the kernels of ONE coupled step on `st` (same arguments every step: the
+// ping-pong parity, dt, t, halt live in the device control block)
+template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev = nullptr)
+{
+    PedArgs<T> pa = ped_args<T>(s);
+    for (int e = 0; e < s->prm.n_exit_cells; ++e) { pa.exit_i[e] = s->exit_i[e]; pa.exit_j[e] = s->exit_j[e]; }
+    pa.n_exit = s->prm.n_exit_cells;
+    int k = 0;
+    auto mark = [&]() { if (ev) cudaEventRecord(ev[k++], st); };     // profiling mode only
+    if (s->np > 0) {
+        const int nb = (s->np + 255) / 256;
+        mark();
+        ped_bin_count_kernel<T><<<nb, 256, 0, st>>>(pa, 1);
+        const int n_items = s->nbins + 1;
+        mark();
+        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, st>>>(s->count, s->start, n_items, s->scan_status, s->ctl);
+        mark();
+        ped_scatter_kernel<T><<<nb, 256, 0, st>>>(pa);
+        mark();
+        ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, st>>>(pa);
+    } else k = 4;
+    FloodArgs<T> fa = flood_args<T>(s);
+    mark();
+    if (s->flood_variant == 1) {
+        dim3 grid((s->grid.nx + TX - 1) / TX, (s->grid.ny + TY - 1) / TY);
+        flood_tile_kernel<T><<<grid, FLOOD_TILE_THREADS, sizeof(TileSmem<T>), st>>>(fa);
+    } else {
+        dim3 blk(32, 8), grid((s->grid.nx + 31) / 32, (s->grid.ny + 7) / 8);
+        flood_cell_kernel<T><<<grid, blk, 0, st>>>(fa);
+    }
+    mark();
+    tail_kernel<T><<<1, 32, 0, st>>>(tail_args<T>(s), 0);
+    mark();
+    CU(cudaGetLastError());
+    return SIM_OK;
+}
+
+// n steps launched kernel by kernel with an event before each launch: per-kernel device time
+template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
+{
+    constexpr int NE = 7, BATCH = 64;
+    std::vector<cudaEvent_t> ev(NE * BATCH);
+    for (auto &e : ev) CU(cudaEventCreate(&e));
+    for (int k = 0; k < 8; ++k) ms[k] = 0.0;
+    int rc = SIM_OK;
+    while (n > 0 && rc == SIM_OK) {
+        const int m = (int)(n < BATCH ? n : BATCH);
+        for (int i = 0; i < m && rc == SIM_OK; ++i) rc = enqueue_step<T>(s, s->stream, &ev[(size_t)i * NE]);
+        if (rc != SIM_OK) break;
+        cudaError_t e = cudaStreamSynchronize(s->stream);
+        if (e != cudaSuccess) { rc = fail(s, SIM_ECUDA, cudaGetErrorString(e)); break; }
+        const int first = s->np > 0 ? 0 : 4;
+        for (int i = 0; i < m; ++i)
+            for (int k = first; k < NE - 1; ++k) {
+                float t = 0.f;
+                cudaEventElapsedTime(&t, ev[(size_t)i * NE + k], ev[(size_t)i * NE + k + 1]);
+                ms[k] += t;
+            }
+        n -= m;
+    }
+    for (auto &e : ev) cudaEventDestroy(e);
+    return rc;
+}
+
+void drop_graphs(sim *s)
+{
+    if (s->graph1) cudaGraphExecDestroy(s->graph1);
+    if (s->graphN) cudaGraphExecDestroy(s->graphN);
+    s->graph1 = s->graphN = nullptr;
+}
+
+template <typename T> int build_graphs(sim *s)
+{
+    for (int which = 0; which < 2; ++which) {
+        const int reps = which ? GRAPH_CHUNK : 1;
+        cudaGraph_t g = nullptr;
+        CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+        int rc = SIM_OK;
+        for (int r = 0; r < reps && rc == SIM_OK; ++r) rc = enqueue_step<T>(s, s->cap_stream);
+        cudaError_t e = cudaStreamEndCapture(s->cap_stream, &g);
+        if (rc != SIM_OK) { if (g) cudaGraphDestroy(g); return rc; }
+        if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+        cudaGraphExec_t ex = nullptr;
+        e = cudaGraphInstantiate(&ex, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
+        (which ? s->graphN : s->graph1) = ex;
+    }
+    return SIM_OK;
+}
+
+template <typename T> int refresh_dt(sim *s)      // lambda of the state in place -> dt, q_in, halt
+{
+    flood_lambda_kernel<T><<<592, 256, 0, s->stream>>>(flood_args<T>(s));
+    tail_kernel<T><<<1, 32, 0, s->stream>>>(tail_args<T>(s), 1);
+    CU(cudaGetLastError());
+    return SIM_OK;
+}
+
+template <typename T> int set_smem_attr(sim *s)
+{
+    CU(cudaFuncSetAttribute(flood_tile_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<T>)));
+    return SIM_OK;
+}
+
+#define DISPATCH(s, fn, ...) ((s)->grid.real_bits == 64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
+
+int copy_out(sim *s, void *dst, const void *src, size_t bytes)
+{
+    if (!dst || !bytes) return SIM_OK;
+    CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, s->stream));
+    return SIM_OK;
+}
+
+int upload(sim *s, void *dst, const void *src, size_t bytes)
+{
+    if (!bytes) return SIM_OK;
+    if (src) CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s->stream));
+    else CU(cudaMemsetAsync(dst, 0, bytes, s->stream));
+    return SIM_OK;
+}
+
+// host-side preparation of one real array with solids applied
+template <typename T>
+void make_zs(const T *z, const uint8_t *mask, size_t n, std::vector<T> &out)
+{
+    out.resize(n);
+    for (size_t c = 0; c < n; ++c) out[c] = (mask && mask[c]) ? (T)INFINITY : z[c];
+}
+
+template <typename T>
+void make_q(const T *h0, const T *u0, const uint8_t *mask, size_t n, std::vector<T> &out)
+{
+    out.assign(n, (T)0);
+    if (h0 && u0)
+        for (size_t c = 0; c < n; ++c) out[c] = (mask && mask[c]) ? (T)0 : h0[c] * u0[c];   // conserved (C8)
+}
+
+template <typename T>
+double default_dt_max(const sim_peds_t *peds, const sim_params_t *p, double dmin)
+{
+    double vm = 1.8;                                        // C10
+    const T *vp = peds ? (const T *)peds->v_pref : nullptr;
+    for (int i = 0; vp && i < peds->n; ++i) if ((double)vp[i] > vm) vm = (double)vp[i];
+    for (int k = 0; k < 4; ++k) if (p->speed_wet[k] > vm) vm = p->speed_wet[k];
+    return std::fmin(1.0, dmin / (p->vmax_factor * vm));
+}
+
+template <typename T>
+int upload_state(sim *s, const sim_topo_t *topo, const void *manning, const sim_peds_t *peds, const sim_params_t *p)
+{
+    const size_t nc = (size_t)s->ncell, rs = sizeof(T);
+    std::vector<T> tmp;
+    make_zs<T>((const T *)topo->z, topo->mask, nc, tmp);
+    if (upload(s, s->zs, tmp.data(), nc * rs)) return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    if (upload(s, s->z0, topo->z, nc * rs)) return SIM_ECUDA;
+    if (upload(s, s->n0, manning, nc * rs)) return SIM_ECUDA;
+    if (upload(s, s->mask, topo->mask, nc)) return SIM_ECUDA;
+    // depth: zero inside solids
+    if (topo->h0) {
+        tmp.resize(nc);
+        const T *h0 = (const T *)topo->h0;
+        for (size_t c = 0; c < nc; ++c) tmp[c] = (topo->mask && topo->mask[c]) ? (T)0 : h0[c];
+        if (upload(s, s->h[0], tmp.data(), nc * rs)) return SIM_ECUDA;
+        CU(cudaStreamSynchronize(s->stream));
+    } else if (upload(s, s->h[0], nullptr, nc * rs)) return SIM_ECUDA;
+    make_q<T>((const T *)topo->h0, (const T *)topo->u0, topo->mask, nc, tmp);
+    if (upload(s, s->qx[0], tmp.data(), nc * rs)) return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    make_q<T>((const T *)topo->h0, (const T *)topo->v0, topo->mask, nc, tmp);
+    if (upload(s, s->qy[0], tmp.data(), nc * rs)) return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    // pedestrians: buffer A in original order
+    const size_t np = (size_t)s->np;
+    if (np) {
+        if (upload(s, s->P[0].x, peds->x, np * rs) || upload(s, s->P[0].y, peds->y, np * rs) ||
+            upload(s, s->P[0].vx, peds->vx, np * rs) || upload(s, s->P[0].vy, peds->vy, np * rs) ||
+            upload(s, s->P[0].vpref, peds->v_pref, np * rs) || upload(s, s->P[0].role, peds->role, np))
+            return SIM_ECUDA;
+        std::vector<uint8_t> fsm(np), act(np, 1);
+        std::vector<int32_t> id(np), neg(np, -1);
+        for (size_t i = 0; i < np; ++i) {
+            fsm[i] = (peds->role && peds->role[i]) ? SIM_FSM_TO_STORAGE : SIM_FSM_EVACUATE;
+            id[i] = (int32_t)i;
+        }
+        if (upload(s, s->P[0].fsm, fsm.data(), np) || upload(s, s->P[0].active, act.data(), np) ||
+            upload(s, s->P[0].id, id.data(), np * 4) || upload(s, s->cellprev, neg.data(), np * 4))
+            return SIM_ECUDA;
+        CU(cudaStreamSynchronize(s->stream));
+    }
+    (void)p;
+    return SIM_OK;
+}
+
+}  // namespace
+
+// ================================================================================ C ABI
+
+extern "C" int sim_workspace_bytes(const sim_grid_t *grid, int32_t n_peds, const sim_params_t *params, size_t *bytes)
+{
+    sim tmp;
+    if (!bytes) return fail(nullptr, SIM_EINVAL, "bytes is NULL");
+    int rc = derive_sizes(&tmp, grid, n_peds, params);
+    if (rc != SIM_OK) { g_create_error = tmp.err; return rc; }
+    Bump b; b.dry = true;
+    *bytes = layout(&tmp, b);
+    return SIM_OK;
+}
+
+extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const void *manning,
+                          const sim_peds_t *peds, const sim_params_t *p, void *workspace,
+                          void *cuda_stream, sim_t **out)
+{
+    if (!out) return fail(nullptr, SIM_EINVAL, "out is NULL");
+    *out = nullptr;
+    sim *s = new sim;
+    auto bail = [&](int rc) { g_create_error = s->err; sim_destroy(s); return rc; };
+    const int32_t n_peds = peds ? peds->n : 0;
+    int rc = derive_sizes(s, grid, n_peds, p);
+    if (rc != SIM_OK) return bail(rc);
+    if (!topo || !topo->z || !manning) return bail(fail(s, SIM_EINVAL, "z and manning are required"));
+    if (n_peds > 0 && (!peds->x || !peds->y || !peds->vx || !peds->vy || !peds->v_pref))
+        return bail(fail(s, SIM_EINVAL, "pedestrian arrays are required when n > 0"));
+    if (!p->nav_dir) return bail(fail(s, SIM_EINVAL, "nav_dir is required"));
+    if (p->n_cap < 0 || p->n_cap > 255) return bail(fail(s, SIM_EINVAL, "n_cap must be in [0, 255]"));
+    if (p->n_exit_cells > 16) return bail(fail(s, SIM_EINVAL, "at most 16 exit cells"));
+    if (!(p->tau > 0) || !(p->B_s > 0) || !(p->g > 0) || !(p->cfl > 0))
+        return bail(fail(s, SIM_EINVAL, "tau, B_s, g, cfl must be positive"));
+    if (p->exit_target < 0 || p->exit_target >= p->n_targets || p->storage_target < 0 ||
+        p->storage_target >= p->n_targets || p->drop_target < 0 || p->drop_target >= p->n_targets)
+        return bail(fail(s, SIM_EINVAL, "target index out of range"));
+    const int nx = grid->nx, ny = grid->ny;
+    auto cell_ok = [&](int c) { return c >= 0 && c < nx * ny; };
+    for (int e = 0; e < p->n_exit_cells; ++e)
+        if (!cell_ok(p->exit_cells[e])) return bail(fail(s, SIM_EINVAL, "exit cell out of range"));
+    if (!cell_ok(p->storage_cell) || !cell_ok(p->drop_cell)) return bail(fail(s, SIM_EINVAL, "storage/drop cell out of range"));
+    for (int k = 0; k < p->n_line; ++k) {
+        if (!cell_ok(p->line_cells[k])) return bail(fail(s, SIM_EINVAL, "barrier cell out of range"));
+        if (topo->mask && topo->mask[p->line_cells[k]]) return bail(fail(s, SIM_EINVAL, "barrier cell is solid"));
+    }
+    if (p->n_line > 0 && p->n_layers > 0 && p->bags_per_cell_layer < 1)
+        return bail(fail(s, SIM_EINVAL, "bags_per_cell_layer must be >= 1"));
+    std::vector<uint8_t> infl[4];
+    infl[0].assign(ny, 0); infl[1].assign(ny, 0); infl[2].assign(nx, 0); infl[3].assign(nx, 0);
+    s->inflow_length = 0.0;
+    for (int f = 0; f < p->n_inflow_faces; ++f) {
+        const int c = p->inflow_cell[f], side = p->inflow_side[f];
+        if (!cell_ok(c) || side > 3) return bail(fail(s, SIM_EINVAL, "inflow face out of range"));
+        const int i = c % nx, j = c / nx;
+        const bool on_edge = (side == SIM_SIDE_W && i == 0) || (side == SIM_SIDE_E && i == nx - 1) ||
+                             (side == SIM_SIDE_S && j == 0) || (side == SIM_SIDE_N && j == ny - 1);
+        if (!on_edge) return bail(fail(s, SIM_EINVAL, "inflow faces must lie on the domain edge (C14)"));
+        uint8_t &m = infl[side][side < 2 ? j : i];
+        if (m == 255) return bail(fail(s, SIM_EINVAL, "too many inflow faces on one cell side"));
+        m += 1;
+        s->inflow_length += side < 2 ? grid->dy : grid->dx;
+    }
+    for (int k = 1; k < p->n_hydro; ++k)
+        if (!(p->hydro_t[k] > p->hydro_t[k - 1])) return bail(fail(s, SIM_EINVAL, "hydro_t must increase"));
+
+    s->prm = *p;
+    for (int e = 0; e < p->n_exit_cells; ++e) { s->exit_i[e] = p->exit_cells[e] % nx; s->exit_j[e] = p->exit_cells[e] / nx; }
+    if (!(s->prm.dt_max > 0)) {
+        const double dmin = grid->dx < grid->dy ? grid->dx : grid->dy;
+        s->prm.dt_max = grid->real_bits == 64 ? default_dt_max<double>(peds, p, dmin) : default_dt_max<float>(peds, p, dmin);
+    }
+    s->flood_variant = (nx % 4 == 0) ? 1 : 0;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return bail(fail(s, SIM_ECUDA, "no CUDA device: this library has no CPU fallback"));
+    s->stream = (cudaStream_t)cuda_stream;
+    Bump b; b.dry = true;
+    s->ws_bytes = layout(s, b);
+    if (workspace) { s->ws = workspace; s->own_ws = false; }
+    else {
+        if (cudaMalloc(&s->ws, s->ws_bytes) != cudaSuccess) { s->ws = nullptr; return bail(fail(s, SIM_ENOMEM, "cudaMalloc of the workspace failed")); }
+        s->own_ws = true;
+    }
+    b = Bump(); b.dry = false; b.base = (char *)s->ws;
+    layout(s, b);
+    auto run = [&]() -> int {
+        CU(cudaMemsetAsync(s->ws, 0, s->ws_bytes, s->stream));
+        CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+        int r = DISPATCH(s, upload_state, s, topo, manning, peds, p);
+        if (r != SIM_OK) return r;
+        for (int k = 0; k < 4; ++k) if (upload(s, s->inflow[k], infl[k].data(), infl[k].size())) return SIM_ECUDA;
+        if (upload(s, s->nav, p->nav_dir, (size_t)p->n_targets * s->ncell)) return SIM_ECUDA;
+        if (p->n_line && upload(s, s->line_cells, p->line_cells, (size_t)p->n_line * 4)) return SIM_ECUDA;
+        if (p->n_hydro && (upload(s, s->hydro_t, p->hydro_t, (size_t)p->n_hydro * 8) ||
+                           upload(s, s->hydro_q, p->hydro_q, (size_t)p->n_hydro * 8))) return SIM_ECUDA;
+        Ctl c{};
+        c.t = 0.0; c.dt = 0.0; c.t_end = s->prm.t_end; c.dt_max = s->prm.dt_max; c.cfl = s->prm.cfl;
+        c.complete = (p->n_line <= 0 || p->n_layers <= 0) ? 1 : 0;
+        c.scan_epoch = 1;
+        CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        r = DISPATCH(s, set_smem_attr, s);
+        if (r != SIM_OK) return r;
+        r = DISPATCH(s, refresh_dt, s);
+        if (r != SIM_OK) return r;
+        CU(cudaStreamSynchronize(s->stream));
+        return SIM_OK;
+    };
+    rc = run();
+    if (rc != SIM_OK) return bail(rc);
+    *out = s;
+    return SIM_OK;
+}
+
+extern "C" int sim_step(sim_t *s, int64_t n)
+{
+    if (!s) return SIM_EINVAL;
+    if (n < 0) return fail(s, SIM_EINVAL, "negative step count");
+    if (!s->graph1) {
+        int rc = DISPATCH(s, build_graphs, s);
+        if (rc != SIM_OK) return rc;
+    }
+    while (n >= GRAPH_CHUNK) { CU(cudaGraphLaunch(s->graphN, s->stream)); n -= GRAPH_CHUNK; }
+    while (n > 0) { CU(cudaGraphLaunch(s->graph1, s->stream)); n -= 1; }
+    return SIM_OK;
+}
+
+extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
+{
+    if (!s) return SIM_EINVAL;
+    if (n < 0 || !kernel_ms) return fail(s, SIM_EINVAL, "bad arguments");
+    return DISPATCH(s, step_profiled, s, n, kernel_ms);
+}
+
+extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? 6 : 2) : 0; }
+
+extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
+{
+    if (!s) return SIM_EINVAL;
+    if (variant != 0 && variant != 1) return fail(s, SIM_EINVAL, "variant must be 0 or 1");
+    if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");
+    CU(cudaStreamSynchronize(s->stream));
+    s->flood_variant = variant;
+    drop_graphs(s);
+    return SIM_OK;
+}
+
+namespace {
+
+template <typename T> int read_flood_t(sim *s, void *h, void *u, void *v, void *z, void *hr)
+{
+    const size_t bytes = (size_t)s->ncell * sizeof(T);
+    Ctl c;
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    if (u || v || hr) {
+        flood_derive_kernel<T><<<1184, 256, 0, s->stream>>>(flood_args<T>(s), u ? (T *)s->scratch_real[0] : nullptr,
+                                                          v ? (T *)s->scratch_real[1] : nullptr,
+                                                          hr ? (T *)s->scratch_real[2] : nullptr);
+        CU(cudaGetLastError());
+    }
+    if (copy_out(s, h, s->h[c.parity], bytes) || copy_out(s, u, s->scratch_real[0], bytes) ||
+        copy_out(s, v, s->scratch_real[1], bytes) || copy_out(s, hr, s->scratch_real[2], bytes))
+        return SIM_ECUDA;
+    if (z) {
+        // bed with the barrier raised; solid cells report the elevation they were created with
+        std::vector<T> zs(s->ncell), z0(s->ncell);
+        CU(cudaMemcpyAsync(zs.data(), s->zs, bytes, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaMemcpyAsync(z0.data(), s->z0, bytes, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        for (int k = 0; k < s->ncell; ++k) if (std::isinf((double)zs[k])) zs[k] = z0[k];
+        CU(cudaMemcpyAsync(s->scratch_real[0], zs.data(), bytes, cudaMemcpyHostToDevice, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        if (copy_out(s, z, s->scratch_real[0], bytes)) return SIM_ECUDA;
+    }
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+template <typename T> int read_peds_t(sim *s, void *x, void *y, void *vx, void *vy, uint8_t *state, uint8_t *fsm,
+                                      uint8_t *active, int32_t *cell, void *timer)
+{
+    const int np = s->np;
+    if (!np) return SIM_OK;
+    ped_gather_kernel<T><<<(np + 255) / 256, 256, 0, s->stream>>>(
+        ped_soa<T>(s, 0), np, s->grid.nx, (T)(1.0 / s->grid.dx), (T)(1.0 / s->grid.dy), s->grid.ny,
+        (T *)s->ped_out[0], (T *)s->ped_out[1], (T *)s->ped_out[2], (T *)s->ped_out[3],
+        s->ped_out_u8[0], s->ped_out_u8[1], s->ped_out_u8[2], s->ped_out_i32[0], (T *)s->ped_out[4], nullptr);
+    CU(cudaGetLastError());
+    const size_t rb = (size_t)np * sizeof(T);
+    if (copy_out(s, x, s->ped_out[0], rb) || copy_out(s, y, s->ped_out[1], rb) || copy_out(s, vx, s->ped_out[2], rb) ||
+        copy_out(s, vy, s->ped_out[3], rb) || copy_out(s, timer, s->ped_out[4], rb) ||
+        copy_out(s, state, s->ped_out_u8[0], np) || copy_out(s, fsm, s->ped_out_u8[1], np) ||
+        copy_out(s, active, s->ped_out_u8[2], np) || copy_out(s, cell, s->ped_out_i32[0], (size_t)np * 4))
+        return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+template <typename T> int stats_t(sim *s, sim_stats_t *o)
+{
+    CU(cudaMemsetAsync(s->stat_d, 0, 8 * sizeof(double), s->stream));
+    CU(cudaMemsetAsync(s->stat_hist, 0, 8 * sizeof(unsigned long long), s->stream));
+    flood_stats_kernel<T><<<1184, 256, 0, s->stream>>>(flood_args<T>(s), s->stat_d);
+    if (s->np) ped_hist_kernel<T><<<(s->np + 255) / 256, 256, 0, s->stream>>>(ped_soa<T>(s, 0), s->np, s->stat_hist, s->stat_d + 4);
+    CU(cudaGetLastError());
+    double d[8]; unsigned long long hist[8]; Ctl c;
+    CU(cudaMemcpyAsync(d, s->stat_d, sizeof d, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(hist, s->stat_hist, sizeof hist, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    std::memset(o, 0, sizeof *o);
+    o->t = c.t; o->dt = c.dt; o->step = c.step;
+    o->volume = d[0]; o->max_h = d[1]; o->max_hr = d[2];
+    for (int k = 0; k < 6; ++k) o->hist[k] = (int64_t)hist[k];
+    o->neg_depth_clamps = (int64_t)c.neg_clamps; o->clamped_volume = c.clamped_volume;
+    o->cursor = c.cursor; o->layer = c.layer; o->bags = c.bags; o->barrier_complete = c.complete;
+    o->deposits = c.deposits;
+    if (d[3] > 0 || d[4] > 0) return fail(s, SIM_ENOTFINITE, "non-finite depth, discharge or position");
+    return SIM_OK;
+}
+
+template <typename T> int bin_peds_t(sim *s, int32_t *key, int32_t *order, int32_t *start)
+{
+    const int np = s->np;
+    if (np) {
+        PedArgs<T> pa = ped_args<T>(s);
+        const int nb = (np + 255) / 256, n_items = s->nbins + 1;
+        Ctl c;
+        CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        const int halt = c.halt;
+        if (halt) { c.halt = 0; CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream)); }
+        ped_bin_count_kernel<T><<<nb, 256, 0, s->stream>>>(pa, 0);
+        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl);
+        ped_scatter_kernel<T><<<nb, 256, 0, s->stream>>>(pa);
+        ped_key_by_id_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 0), s->key, np, s->ped_out_i32[0]);
+        ped_gather_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 1), np, s->grid.nx, (T)1, (T)1, s->grid.ny,
+            nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, s->ped_out_i32[1]);
+        CU(cudaGetLastError());
+        // the scan consumed a ticket range and an epoch: re-arm them without touching dt
+        CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        c.scan_ticket = 0; c.scan_epoch += 1; c.halt = halt;
+        CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
+        if (copy_out(s, key, s->ped_out_i32[0], (size_t)np * 4) || copy_out(s, order, s->ped_out_i32[1], (size_t)np * 4))
+            return SIM_ECUDA;
+    }
+    if (np == 0) CU(cudaMemsetAsync(s->start, 0, (size_t)(s->nbins + 2) * 4, s->stream));
+    if (copy_out(s, start, s->start, (size_t)(s->nbins + 2) * 4)) return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+template <typename T> int write_flood_t(sim *s, const void *h, const void *qx, const void *qy, const void *z)
+{
+    const size_t nc = (size_t)s->ncell, bytes = nc * sizeof(T);
+    Ctl c;
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    const int p = c.parity;
+    if (h) CU(cudaMemcpyAsync(s->h[p], h, bytes, cudaMemcpyHostToDevice, s->stream));
+    if (qx) CU(cudaMemcpyAsync(s->qx[p], qx, bytes, cudaMemcpyHostToDevice, s->stream));
+    if (qy) CU(cudaMemcpyAsync(s->qy[p], qy, bytes, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    if (z) {
+        std::vector<uint8_t> mask(nc);
+        CU(cudaMemcpyAsync(mask.data(), s->mask, nc, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        std::vector<T> zs;
+        make_zs<T>((const T *)z, mask.data(), nc, zs);
+        CU(cudaMemcpyAsync(s->zs, zs.data(), bytes, cudaMemcpyHostToDevice, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+    }
+    return SIM_OK;
+}
+
+}  // namespace
+
+extern "C" int sim_read_flood(sim_t *s, void *h, void *u, void *v, void *z, void *hr)
+{
+    if (!s) return SIM_EINVAL;
+    return DISPATCH(s, read_flood_t, s, h, u, v, z, hr);
+}
+
+extern "C" int sim_read_conserved(sim_t *s, void *h, void *qx, void *qy)
+{
+    if (!s) return SIM_EINVAL;
+    Ctl c;
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    const size_t bytes = (size_t)s->ncell * real_size(s);
+    if (copy_out(s, h, s->h[c.parity], bytes) || copy_out(s, qx, s->qx[c.parity], bytes) ||
+        copy_out(s, qy, s->qy[c.parity], bytes)) return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+extern "C" int sim_read_occupancy(sim_t *s, uint8_t *np_cell)
+{
+    if (!s) return SIM_EINVAL;
+    if (copy_out(s, np_cell, s->occ, (size_t)s->ncell)) return SIM_ECUDA;
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+extern "C" int sim_read_peds(sim_t *s, void *x, void *y, void *vx, void *vy, uint8_t *state, uint8_t *fsm,
+                             uint8_t *active, int32_t *cell, void *timer)
+{
+    if (!s) return SIM_EINVAL;
+    return DISPATCH(s, read_peds_t, s, x, y, vx, vy, state, fsm, active, cell, timer);
+}
+
+extern "C" int sim_get_stats(sim_t *s, sim_stats_t *out)
+{
+    if (!s) return SIM_EINVAL;
+    if (!out) return fail(s, SIM_EINVAL, "out is NULL");
+    return DISPATCH(s, stats_t, s, out);
+}
+
+extern "C" int sim_bin_peds(sim_t *s, int32_t *key, int32_t *order, int32_t *start,
+                            int32_t *n_bins_x, int32_t *n_bins_y, int32_t *k)
+{
+    if (!s) return SIM_EINVAL;
+    if (n_bins_x) *n_bins_x = s->nbx;
+    if (n_bins_y) *n_bins_y = s->nby;
+    if (k) *k = s->kbin;
+    if (!key && !order && !start) return SIM_OK;
+    return DISPATCH(s, bin_peds_t, s, key, order, start);
+}
+
+extern "C" int sim_write_flood(sim_t *s, const void *h, const void *qx, const void *qy, const void *z)
+{
+    if (!s) return SIM_EINVAL;
+    return DISPATCH(s, write_flood_t, s, h, qx, qy, z);
+}
+
+extern "C" int sim_write_peds(sim_t *s, const void *x, const void *y, const void *vx, const void *vy,
+                              const uint8_t *fsm, const uint8_t *active, const void *timer)
+{
+    if (!s) return SIM_EINVAL;
+    const size_t np = (size_t)s->np, rb = np * real_size(s);
+    if (!np) return SIM_OK;
+    // put buffer A back into original order first, so that index i means agent i again
+    CU(cudaStreamSynchronize(s->stream));
+    int rc = sim_read_peds(s, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+    if (rc != SIM_OK) return rc;
+    // ped_out_* now hold x y vx vy timer / state fsm active in original order
+    auto put = [&](void *dst, const void *host, const void *dev_orig, size_t bytes) -> int {
+        if (host) CU(cudaMemcpyAsync(dst, host, bytes, cudaMemcpyHostToDevice, s->stream));
+        else CU(cudaMemcpyAsync(dst, dev_orig, bytes, cudaMemcpyDeviceToDevice, s->stream));
+        return SIM_OK;
+    };
+    // vpref / role / id need un-permuting too: do it on the host (test hook, not hot)
+    std::vector<int32_t> id(np);
+    std::vector<char> vp(rb), vp2(rb);
+    std::vector<uint8_t> role(np), role2(np);
+    CU(cudaMemcpyAsync(id.data(), s->P[0].id, np * 4, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(vp.data(), s->P[0].vpref, rb, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(role.data(), s->P[0].role, np, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    const size_t rs = real_size(s);
+    for (size_t k = 0; k < np; ++k) { std::memcpy(&vp2[(size_t)id[k] * rs], &vp[k * rs], rs); role2[id[k]] = role[k]; }
+    for (size_t k = 0; k < np; ++k) id[k] = (int32_t)k;
+    if (put(s->P[0].x, x, s->ped_out[0], rb) || put(s->P[0].y, y, s->ped_out[1], rb) ||
+        put(s->P[0].vx, vx, s->ped_out[2], rb) || put(s->P[0].vy, vy, s->ped_out[3], rb) ||
+        put(s->P[0].timer, timer, s->ped_out[4], rb) || put(s->P[0].state, nullptr, s->ped_out_u8[0], np) ||
+        put(s->P[0].fsm, fsm, s->ped_out_u8[1], np) || put(s->P[0].active, active, s->ped_out_u8[2], np))
+        return SIM_ECUDA;
+    CU(cudaMemcpyAsync(s->P[0].vpref, vp2.data(), rb, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaMemcpyAsync(s->P[0].role, role2.data(), np, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaMemcpyAsync(s->P[0].id, id.data(), np * 4, cudaMemcpyHostToDevice, s->stream));
+    // occupancy bookkeeping restarts from scratch
+    CU(cudaMemsetAsync(s->occ, 0, (size_t)s->ncell, s->stream));
+    CU(cudaMemsetAsync(s->cellprev, 0xff, np * 4, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+extern "C" int sim_set_time(sim_t *s, double t, double dt)
+{
+    if (!s) return SIM_EINVAL;
+    Ctl c;
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    c.t = t; c.dt = dt; c.halt = (t >= c.t_end) ? 1 : 0;
+    // same piecewise-linear lookup as the tail kernel, on the host copy of the table
+    double q = 0.0;
+    const int n = s->n_hydro;
+    if (n > 0) {
+        std::vector<double> ht(n), hq(n);
+        CU(cudaMemcpyAsync(ht.data(), s->hydro_t, (size_t)n * 8, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaMemcpyAsync(hq.data(), s->hydro_q, (size_t)n * 8, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+        if (t <= ht[0]) q = hq[0];
+        else { q = hq[n - 1]; for (int k = 0; k + 1 < n; ++k) if (t < ht[k + 1]) { q = hq[k] + (hq[k + 1] - hq[k]) * (t - ht[k]) / (ht[k + 1] - ht[k]); break; } }
+    }
+    c.q_in = s->inflow_length > 0 ? q / s->inflow_length : 0.0;
+    CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+extern "C" int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete)
+{
+    if (!s) return SIM_EINVAL;
+    Ctl c;
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    c.cursor = cursor; c.layer = layer; c.bags = bags; c.complete = complete;
+    CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    return SIM_OK;
+}
+
+extern "C" const char *sim_last_error(const sim_t *s) { return s ? s->err.c_str() : g_create_error.c_str(); }
+
+extern "C" void sim_destroy(sim_t *s)
+{
+    if (!s) return;
+    if (s->ws) cudaStreamSynchronize(s->stream);
+    drop_graphs(s);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
+    if (s->own_ws && s->ws) cudaFree(s->ws);
+    delete s;
+}

@@ -1,0 +1,390 @@
+// peds.cuh -- steps (B), (P), (O), (S) and the scalar tail (T) of include/floodped.h.
+//
+// Pedestrians are stored SoA and re-sorted by bin every step (counting sort): this replaces
+// FLAMEGPU's navigation-agent / spatially partitioned messages.  Bins are k x k
+// flood cells with k dx >= R_int, so the 3 x 3 adjacent bins hold every interaction partner
+// (C26); the three bins of one bin-row are contiguous in the sorted order, so the
+// neighbourhood is three contiguous index ranges.
+#pragma once
+
+#include "common.cuh"
+
+namespace fp {
+
+template <typename T>
+struct PedSoA {
+    T *x, *y, *vx, *vy, *vpref, *timer;
+    uint8_t *role, *fsm, *state, *active;
+    int32_t *id;
+    int32_t *cell;                   // level-n containing cell (valid in the sorted buffer)
+};
+
+template <typename T>
+struct PedArgs {
+    int n;                           // all agents, active or not
+    int nx, ny, kbin, nbx, nby, nbins;
+    T inv_dx, inv_dy, dxk;
+    T h_dry, hr_edge[3], speed_wet[4];
+    T inv_tau, A_s, inv_B, two_r, R_int, vmax_factor, t_pick, t_drop;
+    int n_targets, exit_target, storage_target, drop_target;
+    int n_exit; int exit_i[16], exit_j[16];
+    int storage_i, storage_j, drop_i, drop_j, arrive;
+    PedSoA<T> A, B;                  // A: level n (any order) and level n+1; B: level n sorted by bin
+    int32_t *key, *off;              // per slot of A: bin key, rank inside the bin
+    int32_t *count;                  // [nbins+1] (zeroed by the scan after use)
+    int32_t *start;                  // [nbins+2] exclusive scan
+    int32_t *cellprev;               // per slot: cell whose occupancy this slot set last step, or -1
+    uint8_t *occ;                    // [ncell] N_p of the current step, saturated at 255
+    const uint8_t *mask;             // [ncell] 1 = solid
+    const uint8_t *nav;              // [n_targets][ncell]
+    const T *h[2], *qx[2], *qy[2];   // flood state (level n is [ctl->parity])
+    Ctl *ctl;
+};
+
+template <typename T> __device__ __forceinline__ int cell_of(T x, T inv, int n)
+{
+    int i = (int)floor(mul_rn(x, inv));
+    return min(max(i, 0), n - 1);
+}
+
+// ---------------------------------------------------------------------------------- (B) count
+// Key of every agent and its rank inside the bin.  Agents arrive nearly sorted (last step's
+// order), so lanes of a warp mostly share a key: one atomic per distinct key per warp
+// (warp-aggregated atomics via match.any).  Also clears the occupancy set by the previous step.
+template <typename T>
+__global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int clear_occ)
+{
+    if (a.ctl->halt) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= a.n) return;
+    const unsigned lanes = __activemask();
+    int key = a.nbins, cell = -1;
+    if (a.A.active[s]) {
+        const int ix = cell_of(a.A.x[s], a.inv_dx, a.nx), iy = cell_of(a.A.y[s], a.inv_dy, a.ny);
+        cell = iy * a.nx + ix;
+        key = (iy / a.kbin) * a.nbx + ix / a.kbin;
+    }
+    const unsigned peers = __match_any_sync(lanes, key);
+    const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&a.count[key], __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    a.key[s] = key;
+    a.off[s] = base + __popc(peers & ((1u << lane) - 1u));
+    a.A.cell[s] = cell;
+    if (clear_occ) {
+        const int c = a.cellprev[s];
+        if (c >= 0) a.occ[c] = 0;      // sparse clear: only cells that were set (no dense memset)
+    }
+}
+
+// ---------------------------------------------------------------------------------- (B) scan
+// Single-pass exclusive scan with decoupled look-back over tiles of SCAN_TILE counts.
+// status word = (epoch*4 + flag) << 32 | value; flag 1 = tile aggregate, 2 = inclusive prefix.
+// The epoch (one per executed step) makes stale flags of earlier steps read as "not ready", so
+// the status array never needs clearing.  Also zeroes count[] for the next step and writes
+// start[n_items] = total.
+constexpr int SCAN_THREADS = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_bins_kernel(int32_t *count, int32_t *start, int n_items,
+                                                                 unsigned long long *status, Ctl *ctl)
+{
+    __shared__ int warp_sum[SCAN_THREADS / 32];
+    __shared__ int tile_s, excl_s;
+    if (ctl->halt) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) tile_s = (int)atomicAdd(&ctl->scan_ticket, 1u);
+    __syncthreads();
+    const int tile = tile_s;
+    const unsigned epoch = ctl->scan_epoch;
+    const int base = tile * SCAN_TILE + tid * SCAN_ITEMS;
+    int v[SCAN_ITEMS], sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        const int i = base + k;
+        v[k] = i < n_items ? count[i] : 0;
+        if (i < n_items) count[i] = 0;
+        sum += v[k];
+    }
+    int inc = sum;                                    // inclusive scan of thread sums in the warp
+    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) warp_sum[warp] = inc;
+    __syncthreads();
+    int warp_off = 0, tile_total = 0;
+#pragma unroll
+    for (int w = 0; w < SCAN_THREADS / 32; ++w) { const int ws = warp_sum[w]; if (w < warp) warp_off += ws; tile_total += ws; }
+    // publish the aggregate, then look back (warp 0)
+    if (warp == 0) {
+        const unsigned long long tag = (unsigned long long)(epoch * 4u);
+        if (lane == 0) {
+            const unsigned long long w = ((tag + (tile == 0 ? 2ull : 1ull)) << 32) | (unsigned)tile_total;
+            atomicExch(&status[tile], w);
+        }
+        int excl = 0;
+        if (tile > 0) {
+            int look = tile - 1;
+            while (true) {
+                const int idx = look - lane;
+                unsigned long long w = 0; unsigned flag = 0;
+                do {
+                    if (idx >= 0) {
+                        w = *((volatile unsigned long long *)&status[idx]);
+                        const unsigned hi = (unsigned)(w >> 32);
+                        flag = (hi >> 2) == epoch ? (hi & 3u) : 0u;
+                    } else flag = 2u, w = 0;          // before tile 0: prefix 0
+                } while (__any_sync(0xffffffffu, flag == 0u));
+                const unsigned done = __ballot_sync(0xffffffffu, flag == 2u);
+                const int first_done = done ? __ffs(done) - 1 : 32;
+                int val = lane <= first_done ? (int)(unsigned)(w & 0xffffffffull) : 0;
+                for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
+                excl += val;
+                if (done) break;
+                look -= 32;
+            }
+            if (lane == 0) {
+                const unsigned long long w = ((tag + 2ull) << 32) | (unsigned)(excl + tile_total);
+                atomicExch(&status[tile], w);
+            }
+        }
+        if (lane == 0) excl_s = excl;
+    }
+    __syncthreads();
+    int run = excl_s + warp_off + (inc - sum);
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        const int i = base + k;
+        if (i < n_items) start[i] = run;
+        run += v[k];
+        if (i == n_items - 1) start[n_items] = run;
+    }
+}
+
+// ---------------------------------------------------------------------------------- (B) scatter
+template <typename T>
+__global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
+{
+    if (a.ctl->halt) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= a.n) return;
+    const int d = a.start[a.key[s]] + a.off[s];
+    a.B.x[d] = a.A.x[s]; a.B.y[d] = a.A.y[s]; a.B.vx[d] = a.A.vx[s]; a.B.vy[d] = a.A.vy[s];
+    a.B.vpref[d] = a.A.vpref[s]; a.B.timer[d] = a.A.timer[s];
+    a.B.role[d] = a.A.role[s]; a.B.fsm[d] = a.A.fsm[s]; a.B.state[d] = a.A.state[s];
+    a.B.active[d] = a.A.active[s]; a.B.id[d] = a.A.id[s]; a.B.cell[d] = a.A.cell[s];
+}
+
+// ---------------------------------------------------------------------------------- (P)+(O)
+// One thread per sorted slot d: reads level n from B (+ flood level n), writes level n+1 to A[d].
+template <typename T>
+__global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
+{
+    if (a.ctl->halt) return;
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d >= a.n) return;
+    const PedSoA<T> &B = a.B, &A = a.A;
+    const T x = B.x[d], y = B.y[d], vx = B.vx[d], vy = B.vy[d], vpref = B.vpref[d];
+    T timer = B.timer[d];
+    const uint8_t role = B.role[d], act = B.active[d];
+    uint8_t fsm = B.fsm[d], state = B.state[d];
+    const int c = B.cell[d];
+    A.vpref[d] = vpref; A.role[d] = role; A.id[d] = B.id[d];
+    if (!act) {
+        A.x[d] = x; A.y[d] = y; A.vx[d] = vx; A.vy[d] = vy; A.timer[d] = timer;
+        A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 0;
+        a.cellprev[d] = -1;
+        return;
+    }
+    const int ix = c % a.nx, iy = c / a.nx;
+    const int bx = ix / a.kbin, by = iy / a.kbin;
+
+    // 4. social repulsion over the 3 x 3 adjacent bins (C24, C26) + N_p of my cell
+    T ax = T(0), ay = T(0);
+    int same = 0, lower = 0;
+    for (int jy = max(by - 1, 0); jy <= min(by + 1, a.nby - 1); ++jy) {
+        const int s0 = a.start[jy * a.nbx + max(bx - 1, 0)];
+        const int s1 = a.start[jy * a.nbx + min(bx + 1, a.nbx - 1) + 1];
+        for (int j = s0; j < s1; ++j) {
+            const T ddx = x - B.x[j], ddy = y - B.y[j];
+            const T dist = real_sqrt(ddx * ddx + ddy * ddy);
+            if (dist > T(0) && dist < a.R_int) {
+                const T f = a.A_s * real_exp((a.two_r - dist) * a.inv_B) / dist;
+                ax += f * ddx; ay += f * ddy;
+            }
+            if (jy == by && B.cell[j] == c) { same += 1; lower += (j < d); }
+        }
+    }
+    // (O) one agent per occupied cell publishes N_p; remember the cell for next step's clear
+    if (lower == 0) a.occ[c] = (uint8_t)min(same, 255);
+    a.cellprev[d] = c;
+
+    // 8. exit (C29): level-n cell within arrive_cells of an exit cell
+    if (role == 0 || fsm == 0) {
+        bool out = false;
+        for (int e = 0; e < a.n_exit; ++e)
+            out |= max(abs(ix - a.exit_i[e]), abs(iy - a.exit_j[e])) <= a.arrive;
+        if (out) {
+            A.x[d] = x; A.y[d] = y; A.vx[d] = vx; A.vy[d] = vy; A.timer[d] = timer;
+            A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 0;
+            return;
+        }
+    }
+    // 1. sample U^n at the containing cell -> HR -> Table 1 (C17-C20)
+    const int p = a.ctl->parity;
+    const T h = a.h[p][c];
+    T u = T(0), v = T(0);
+    if (h > a.h_dry) { u = div_rn(a.qx[p][c], h); v = div_rn(a.qy[p][c], h); }
+    const T hr = mul_rn(add_rn(fmax(fabs(u), fabs(v)), T(0.5)), h);
+    if (!(h > a.h_dry)) state = 0;
+    else if (hr < a.hr_edge[0]) state = 1;
+    else if (hr < a.hr_edge[1]) state = 2;
+    else if (hr < a.hr_edge[2]) state = 3;
+    else state = 4;
+    // 2. desired speed
+    T v0 = state == 0 ? vpref : a.speed_wet[state - 1];
+    if (fsm == 2 || fsm == 4) v0 = T(0);
+    // 3. desired direction from the navigation field of the current target
+    int target = a.exit_target;
+    if (fsm == 1) target = a.storage_target; else if (fsm == 3) target = a.drop_target;
+    const int code = a.nav[(size_t)target * ((size_t)a.nx * a.ny) + c];
+    T ex = T(0), ey = T(0);
+    if (code < 8) {
+        const T r = T(0.70710678118654752440);
+        const int dxs = (code == 0 || code == 1 || code == 7) - (code == 3 || code == 4 || code == 5);
+        const int dys = (code == 1 || code == 2 || code == 3) - (code == 5 || code == 6 || code == 7);
+        const T m = (dxs != 0 && dys != 0) ? r : T(1);
+        ex = m * T(dxs); ey = m * T(dys);
+    }
+    // 5. velocity: backward Euler on the relaxation term (C25), speed cap
+    const T dt = (T)a.ctl->dt;
+    const T den = T(1) / (T(1) + dt * a.inv_tau);
+    T wx = (vx + dt * (v0 * ex * a.inv_tau + ax)) * den;
+    T wy = (vy + dt * (v0 * ey * a.inv_tau + ay)) * den;
+    const T wmax = a.vmax_factor * v0, wn = real_sqrt(wx * wx + wy * wy);
+    if (wn > wmax) { const T f = wn > T(0) ? wmax / wn : T(0); wx *= f; wy *= f; }
+    // 6. move, axis by axis, rejecting moves into solids or out of the domain (C27)
+    auto blocked = [&](T px, T py) {
+        const T fi = floor(mul_rn(px, a.inv_dx)), fj = floor(mul_rn(py, a.inv_dy));
+        if (fi < T(0) || fi >= T(a.nx) || fj < T(0) || fj >= T(a.ny)) return true;
+        return a.mask[(int)fj * a.nx + (int)fi] != 0;
+    };
+    T xn = x + dt * wx, yn = y;
+    if (blocked(xn, yn)) { xn = x; wx = T(0); }
+    yn = y + dt * wy;
+    if (blocked(xn, yn)) { yn = y; wy = T(0); }
+    // 7. responder FSM on the level-n cell (C31)
+    if (role == 1) {
+        if (fsm == 1) {
+            if (max(abs(ix - a.storage_i), abs(iy - a.storage_j)) <= a.arrive) { fsm = 2; timer = a.t_pick; }
+        } else if (fsm == 2) {
+            timer = add_rn(timer, -dt);
+            if (timer <= T(0)) fsm = 3;
+        } else if (fsm == 3) {
+            if (max(abs(ix - a.drop_i), abs(iy - a.drop_j)) <= a.arrive) { fsm = 4; timer = a.t_drop; }
+        } else if (fsm == 4) {
+            timer = add_rn(timer, -dt);
+            if (timer <= T(0)) { atomicAdd(&a.ctl->D, 1); fsm = a.ctl->complete ? 0 : 1; }
+        }
+    }
+    A.x[d] = xn; A.y[d] = yn; A.vx[d] = wx; A.vy[d] = wy; A.timer[d] = timer;
+    A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 1;
+}
+
+// ---------------------------------------------------------------------------------- (S)+(T) tail
+// One thread: sandbag arithmetic, time, next dt, next inflow.
+template <typename T>
+struct TailArgs {
+    Ctl *ctl;
+    T *zs;
+    const int32_t *line_cells;
+    int n_line, bags_per_cell_layer, n_layers;
+    T layer_thickness;
+    const double *hydro_t, *hydro_q;
+    int n_hydro;
+    double inv_inflow_length;
+};
+
+__device__ __forceinline__ double hydrograph(const double *t, const double *q, int n, double time)
+{
+    if (n <= 0) return 0.0;
+    if (time <= t[0]) return q[0];
+    for (int k = 0; k + 1 < n; ++k)
+        if (time < t[k + 1]) return q[k] + (q[k + 1] - q[k]) * (time - t[k]) / (t[k + 1] - t[k]);
+    return q[n - 1];
+}
+
+// first = 1: only derive dt and q_in from the state already in place (create / test hooks)
+template <typename T>
+__global__ void tail_kernel(TailArgs<T> a, int first)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    Ctl *c = a.ctl;
+    if (!first) {
+        if (c->halt) return;
+        const int D = c->D;
+        c->deposits += D;
+        for (int d = 0; d < D && !c->complete; ++d) {
+            c->bags += 1;
+            if (c->bags == a.bags_per_cell_layer) {
+                a.zs[a.line_cells[c->cursor]] += a.layer_thickness;
+                c->bags = 0; c->cursor += 1;
+                if (c->cursor == a.n_line) { c->layer += 1; c->cursor = 0; }
+                if (c->layer == a.n_layers) c->complete = 1;
+            }
+        }
+        c->D = 0;
+        c->t += c->dt;
+        c->step += 1;
+        c->parity ^= 1;
+        c->scan_epoch += 1;
+    }
+    const double lam = __longlong_as_double((long long)c->lam_bits);
+    double dt = c->dt_max;
+    if (lam > 0.0) dt = fmin(dt, c->cfl / lam);
+    if (c->t + dt > c->t_end) dt = fmax(0.0, c->t_end - c->t);
+    c->dt = dt;
+    c->lam_bits = 0ull;
+    c->scan_ticket = 0u;
+    c->halt = (c->t >= c->t_end) ? 1 : 0;
+    c->q_in = hydrograph(a.hydro_t, a.hydro_q, a.n_hydro, c->t) * a.inv_inflow_length;
+}
+
+// ---------------------------------------------------------------------------------- read-back
+// un-permute to original index order ("coordinates and states of the pedestrian agents")
+template <typename T>
+__global__ void ped_gather_kernel(PedSoA<T> A, int n, int nx, T inv_dx, T inv_dy, int ny,
+                                  T *x, T *y, T *vx, T *vy, uint8_t *state, uint8_t *fsm,
+                                  uint8_t *active, int32_t *cell, T *timer, int32_t *order)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int i = A.id[s];
+    if (x) x[i] = A.x[s];
+    if (y) y[i] = A.y[s];
+    if (vx) vx[i] = A.vx[s];
+    if (vy) vy[i] = A.vy[s];
+    if (state) state[i] = A.state[s];
+    if (fsm) fsm[i] = A.fsm[s];
+    if (active) active[i] = A.active[s];
+    if (cell) cell[i] = cell_of(A.y[s], inv_dy, ny) * nx + cell_of(A.x[s], inv_dx, nx);
+    if (timer) timer[i] = A.timer[s];
+    if (order) order[s] = i;
+}
+
+template <typename T>
+__global__ void ped_key_by_id_kernel(PedSoA<T> A, const int32_t *key, int n, int32_t *key_by_id)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) key_by_id[A.id[s]] = key[s];
+}
+
+// state histogram for sim_get_stats: hist[0..4] active by state, hist[5] = left the domain
+template <typename T>
+__global__ void ped_hist_kernel(PedSoA<T> A, int n, unsigned long long *hist, double *n_bad)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    atomicAdd(&hist[A.active[s] ? min((int)A.state[s], 4) : 5], 1ull);
+    if (!isfinite((double)A.x[s]) || !isfinite((double)A.y[s])) atomicAdd(n_bad, 1.0);
+}
+
+}  // namespace fp

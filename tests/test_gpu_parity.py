@@ -1,0 +1,286 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+one step from identical injected state; integers bit-exact, floats within the stated tolerance
+(1e-12 fp64, 1e-5 fp32 in the mixed norm, BASELINE.json north_star); multi-step aggregates."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1908_05232_b200 import binding, scenarios as S
+from helpers import box
+from gpu_common import make_pair, sync, mixed, rounded
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: 1e-12, 32: 1e-5}
+
+
+def _compare_flood(o, g, bits):
+    a, b = g.read_conserved(), o.read_conserved()
+    for k in ("h", "qx", "qy"):
+        assert mixed(a[k], b[k]) <= TOL[bits], (k, mixed(a[k], b[k]))
+    sa, sb = g.stats(), o.stats()
+    assert abs(sa["dt"] - sb["dt"]) <= 10 * TOL[bits] * sb["dt"]
+    assert abs(sa["t"] - sb["t"]) <= 1e-12 * max(sb["t"], 1.0)
+    assert sa["neg_depth_clamps"] == sb["neg_depth_clamps"]
+
+
+def _ped_compare(o, g, sc, p_before, dt, dep_before=(0, 0)):
+    """integers exact; floats within tolerance except where a float decides a discontinuous
+    choice within rounding of its threshold (interaction cut-off, cell edge) -- those agents are
+    listed and must be very few."""
+    bits = sc.real_bits
+    a, b = g.read_peds(), o.read_peds()
+    assert np.array_equal(a["active"], b["active"])
+    act = b["active"] == 1
+    assert np.array_equal(a["fsm"], b["fsm"])
+    assert np.array_equal(a["state"][act], b["state"][act])
+    assert np.array_equal(a["timer"][act].astype(np.float64), rounded(b["timer"][act], g.real))
+    # agents with a partner within rounding of the cut-off, or landing within rounding of a cell edge
+    x0, y0 = p_before["x"], p_before["y"]
+    was = p_before["active"] == 1
+    skip = np.zeros(sc.n_peds, bool)
+    idx = np.flatnonzero(was)
+    if idx.size and idx.size <= 20000:
+        from scipy.spatial import cKDTree
+        t = cKDTree(np.c_[x0[idx], y0[idx]])
+        for i, j in t.query_pairs(sc.R_int * (1 + 1e-5)):
+            d = math.hypot(x0[idx[i]] - x0[idx[j]], y0[idx[i]] - y0[idx[j]])
+            if abs(d - sc.R_int) < 1e-5 * sc.R_int:
+                skip[idx[i]] = skip[idx[j]] = True
+    for arr, d in ((b["x"], sc.dx), (b["y"], sc.dy)):
+        f = arr / d
+        skip |= np.abs(f - np.round(f)) < 1e-5
+    # every agent NOT near such a threshold must agree; those near one may take the other branch
+    bad = np.zeros(sc.n_peds, bool)
+    for k in ("x", "y", "vx", "vy"):
+        scale = max(float(np.max(np.abs(b[k][act]))) if act.any() else 0.0, 1e-300)
+        bad |= act & (np.abs(a[k] - b[k]) > TOL[bits] * scale)
+    bad |= act & (a["cell"] != b["cell"])
+    assert not np.any(bad & ~skip), (np.flatnonzero(bad & ~skip)[:10], int(bad.sum()))
+    assert bad.sum() <= max(2, sc.n_peds // 200), int(bad.sum())
+    sa, sb = g.stats(), o.stats()
+    assert sa["deposits"] - dep_before[1] == sb["deposits"] - dep_before[0] and sa["hist"][5] == sb["hist"][5]
+    assert (sa["cursor"], sa["layer"], sa["bags"], sa["barrier_complete"]) == (sb["cursor"], sb["layer"], sb["bags"], sb["barrier_complete"])
+
+
+def _one_step(sc, evolve, variant=None, check_peds=True):
+    o, g = make_pair(sc, evolve=evolve, variant=variant)
+    if not evolve:
+        sync(o, g, sc)
+    p0 = o.read_peds()
+    dt = o.stats()["dt"]
+    o.step(1); g.step(1)
+    _compare_flood(o, g, sc.real_bits)
+    if sc.n_peds and check_peds:
+        occ = g.read_occupancy().astype(np.int64)
+        assert np.array_equal(occ, np.minimum(o.read_occupancy(), 255))
+        _ped_compare(o, g, sc, p0, dt)
+    return o, g
+
+
+# ------------------------------------------------------------------ flood, single step
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("evolve", [0, 7, 40])
+def test_config1_single_step_fp64(variant, evolve):
+    _one_step(S.make(1), evolve, variant)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config2_single_step_fp32_wet_dry_inflow(variant):
+    sc = S.make(2)
+    sc.hydro_q = sc.hydro_q * 20.0            # a stronger flood so that a lot of the hall is wet
+    _one_step(sc, 300, variant)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config4_mini_single_step_fp32_buildings_all_hr_classes(variant):
+    sc = S.make(4, n=256, n_peds=5000)
+    o, g = _one_step(sc, 150, variant)
+    hist = o.stats()["hist"]
+    assert hist[1] > 0 and hist[2] > 0 and hist[3] > 0      # low, medium, high all present
+
+
+@pytest.mark.parametrize("nx,ny", [(4, 4), (64, 16), (100, 37), (130, 50), (33, 9), (7, 5)])
+def test_ragged_tiles_and_tiny_grids(nx, ny):
+    rng = np.random.default_rng(nx * 100 + ny)
+    z = 0.2 * rng.random((ny, nx))
+    h0 = np.where(rng.random((ny, nx)) < 0.7, rng.random((ny, nx)), 0.0)
+    mask = (rng.random((ny, nx)) < 0.1).astype(np.uint8)
+    for bits in (64, 32):
+        sc = box(nx, ny, dx=0.5, real_bits=bits, z=z, h0=h0, u0=rng.normal(0, 0.5, (ny, nx)),
+                 v0=rng.normal(0, 0.5, (ny, nx)), mask=mask, manning=0.03, dt_max=0.05)
+        for variant in ((0, 1) if nx % 4 == 0 else (0,)):
+            o, g = make_pair(sc, evolve=0, variant=variant)
+            sync(o, g, sc)
+            for _ in range(3):
+                o.step(1); g.step(1)
+                # re-sync so that each step starts from identical inputs
+                _compare_flood(o, g, bits)
+                sync(o, g, sc)
+
+
+def test_tiled_kernel_rejects_unaligned_width():
+    sc = box(30, 8, dx=1.0, real_bits=32, h0=0.1)
+    g = binding.Sim(sc)
+    with pytest.raises(binding.FloodpedError):
+        g.set_flood_variant(1)
+    g.step(2)
+    assert g.stats()["step"] == 2
+
+
+# ------------------------------------------------------------------ binning, occupancy
+
+@pytest.mark.parametrize("cfg,kw", [(1, {}), (2, {}), (4, dict(n=256, n_peds=20000))])
+def test_binning_bit_exact(cfg, kw):
+    sc = S.make(cfg, **kw)
+    o, g = make_pair(sc, evolve=25)
+    ob, gb = o.binning(), g.bin_peds()
+    nb = ob["nbx"] * ob["nby"]
+    assert (gb["nbx"], gb["nby"], gb["k"]) == (ob["nbx"], ob["nby"], ob["k"])
+    assert np.array_equal(gb["key"], ob["key"])
+    assert np.array_equal(gb["start"][:nb + 1], ob["start"])
+    assert gb["start"][nb + 1] == sc.n_peds                      # inactive agents sort last
+    order = gb["order"]
+    assert np.array_equal(np.sort(order), np.arange(sc.n_peds))  # a permutation
+    assert np.all(np.diff(gb["key"][order]) >= 0)                # sorted by bin; order inside a bin is free
+    # binning twice changes nothing and a following step still agrees with the oracle
+    gb2 = g.bin_peds()
+    assert np.array_equal(gb2["key"], gb["key"]) and np.array_equal(gb2["start"], gb["start"])
+    o.step(1); g.step(1)
+    assert np.array_equal(g.read_peds()["active"], o.read_peds()["active"])
+
+
+# ------------------------------------------------------------------ pedestrians, single step
+
+def test_dense_crowd_single_step_fp64_and_fp32():
+    rng = np.random.default_rng(9)
+    n = 32
+    c = rng.uniform(8, 24, size=(5, 2))
+    pts = np.clip(c[rng.integers(0, 5, 1500)] + rng.normal(0, 1.2, size=(1500, 2)), 0.05, n - 0.05)
+    for bits, dx in ((64, 1.0), (32, 0.5), (32, 0.25)):
+        m = int(n / dx)
+        h0 = np.where(np.arange(m)[None, :] < m // 2, 0.4, 0.0) + np.zeros((m, 1))
+        sc = box(m, m, dx=dx, real_bits=bits, h0=h0, v0=0.9 * (h0 > 0),
+                 peds=dict(x=pts[:, 0], y=pts[:, 1], vx=rng.normal(0, 0.5, 1500), vy=rng.normal(0, 0.5, 1500),
+                           vpref=rng.uniform(0.8, 1.6, 1500)),
+                 exit_cell=(m // 2) * m + m - 1, dt_max=0.05, manning=0.02)
+        _one_step(sc, 0)
+        _one_step(sc, 5)
+
+
+def test_config3_responders_and_barrier_single_steps():
+    sc = S.make(3, n=128, n_evac=300, n_resp=60)
+    sc.t_pick = sc.t_drop = 2.0
+    o, g = make_pair(sc, evolve=0)
+    sync(o, g, sc)
+    for k in range(12):                      # compare at steps 0, 150, 300, ... each from synced state
+        p0 = o.read_peds(); dt = o.stats()["dt"]
+        dep = (o.stats()["deposits"], g.stats()["deposits"])
+        o.step(1); g.step(1)
+        _compare_flood(o, g, 32)
+        _ped_compare(o, g, sc, p0, dt, dep)
+        z_o, z_g = o.read_flood()["z"], g.read_flood(("z",))["z"]
+        assert mixed(z_g, z_o) <= 1e-6
+        o.step(149)
+        sync(o, g, sc)
+    st = o.stats()
+    assert st["deposits"] > 0                # the barrier is actually being built in this window
+
+
+def test_deposits_in_one_step_raise_the_bed_like_the_oracle():
+    sc = S.make(3, n=128, n_evac=50, n_resp=40)
+    o, g = make_pair(sc, evolve=0)
+    sync(o, g, sc)
+    total = 0
+    for rnd_ in range(4):                    # 4 x 40 deposits in single steps: cursor/layer arithmetic
+        for side in (o, g):
+            side.write_peds(fsm=np.r_[np.full(40, 4), np.zeros(50)].astype(np.uint8),
+                            timer=np.r_[np.full(40, 0.01), np.zeros(50)])
+        o.step(1); g.step(1)
+        total += 40
+        a, b = g.stats(), o.stats()
+        assert a["deposits"] == b["deposits"] == total
+        assert (a["cursor"], a["layer"], a["bags"], a["barrier_complete"]) == (b["cursor"], b["layer"], b["bags"], b["barrier_complete"])
+        assert mixed(g.read_flood(("z",))["z"], o.read_flood()["z"]) <= 1e-6
+        assert np.array_equal(g.read_peds()["fsm"], o.read_peds()["fsm"])
+    assert b["layer"] == total // len(sc.line_cells)
+
+
+# ------------------------------------------------------------------ multi-step aggregates
+
+def test_config1_100_steps_aggregates():
+    sc = S.make(1)
+    o = oracle.Oracle(sc); g = binding.Sim(sc)
+    o.step(100); g.step(100)
+    a, b = g.stats(), o.stats()
+    assert a["step"] == b["step"] == 100
+    assert abs(a["volume"] - b["volume"]) <= 1e-10 * b["volume"]
+    assert abs(a["max_h"] - b["max_h"]) <= 1e-9 * b["max_h"]
+    assert abs(a["t"] - b["t"]) <= 1e-10 * b["t"]
+    assert a["neg_depth_clamps"] == 0
+    assert sum(abs(x - y) for x, y in zip(a["hist"], b["hist"])) <= 0.01 * sc.n_peds
+    c, d = g.read_conserved(), o.read_conserved()
+    assert mixed(c["h"], d["h"]) <= 1e-9
+
+
+def test_config2_multi_step_aggregates_fp32():
+    sc = S.make(2)
+    sc.hydro_q = sc.hydro_q * 10.0
+    o = oracle.Oracle(sc); g = binding.Sim(sc)
+    o.step(600); g.step(600)
+    a, b = g.stats(), o.stats()
+    assert abs(a["t"] - b["t"]) <= 1e-4 * b["t"]
+    assert abs(a["volume"] - b["volume"]) <= 1e-4 * b["volume"]      # fp32 storage of h: 1e-5 per DESIGN + dt drift
+    assert abs(a["max_h"] - b["max_h"]) <= 1e-3 * b["max_h"]
+    assert sum(abs(x - y) for x, y in zip(a["hist"], b["hist"])) <= 0.01 * sc.n_peds
+
+
+def test_t_end_lands_and_halts_on_device():
+    sc = S.make(1)
+    sc.t_end = 2.0
+    g = binding.Sim(sc)
+    g.step(200)
+    st = g.stats()
+    assert st["t"] == 2.0 and st["step"] < 200
+    h = g.read_conserved()["h"].copy()
+    g.step(64)
+    assert g.stats()["step"] == st["step"] and np.array_equal(h, g.read_conserved()["h"])
+
+
+def test_no_pedestrians_and_lake_at_rest_on_gpu():
+    sc = S.make(1, n_peds=0)
+    sc.h0 = np.maximum(0.0, 0.2 - sc.z)                 # island
+    for variant in (0, 1):
+        g = binding.Sim(sc); g.set_flood_variant(variant)
+        g.step(500)
+        c = g.read_conserved()
+        assert np.max(np.abs(c["qx"])) <= 1e-12 and np.max(np.abs(c["qy"])) <= 1e-12
+        assert g.kernels_per_step() == 2
+
+
+def test_device_pointer_outputs_and_torch_workspace():
+    import torch
+    sc = S.make(2, n=64, n_evac=200)
+    g = binding.Sim(sc)                                  # state lives in a torch.empty workspace
+    assert g._ws is not None and g._ws.is_cuda
+    g.step(10)
+    host = g.read_conserved()
+    dev = [torch.empty(g.ncell, dtype=torch.float32, device="cuda") for _ in range(3)]
+    g.read_conserved_into(*[t.data_ptr() for t in dev])
+    assert np.array_equal(dev[0].cpu().numpy(), host["h"])
+    g2 = binding.Sim(sc, use_torch_workspace=False)      # library-owned cudaMalloc
+    g2.step(10)
+    assert np.array_equal(g2.read_conserved()["h"], host["h"])
+
+
+def test_not_finite_state_is_reported():
+    sc = S.make(1, n_peds=0)
+    g = binding.Sim(sc)
+    h = np.array(sc.h0, np.float64); h[100] = np.nan
+    g.write_flood(h=h)
+    with pytest.raises(binding.FloodpedError) as e:
+        g.stats()
+    assert e.value.code == binding.SIM_ENOTFINITE
