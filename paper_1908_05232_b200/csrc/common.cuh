@@ -48,15 +48,30 @@ __device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(
 __device__ __forceinline__ float  div_rn(float a, float b)   { return __fdiv_rn(a, b); }
 __device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
 
-__device__ __forceinline__ float  fast_rcp(float a)  { return __frcp_rn(a); }
+// Approximate single-instruction math (MUFU) for the flood kernel's fp32 path: relative error
+// <= 2^-22, far inside the 1e-5 tolerance of the fp32 configs; fp64 stays IEEE.
+__device__ __forceinline__ float  fast_rcp(float a)  { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 __device__ __forceinline__ double fast_rcp(double a) { return 1.0 / a; }
+__device__ __forceinline__ float  fast_sqrt(float a)  { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ double fast_sqrt(double a) { return sqrt(a); }
+__device__ __forceinline__ float  fast_rsqrt(float a)  { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ double fast_rsqrt(double a) { return rsqrt(a); }
+__device__ __forceinline__ float  fast_exp(float a)
+{
+    float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a * 1.4426950408889634f)); return r;
+}
+__device__ __forceinline__ double fast_exp(double a) { return exp(a); }
+// h^(-7/3) for the Manning term, h > h_dry > 0
+__device__ __forceinline__ float  pow_m73(float h)
+{
+    float l, r;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(h));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(l * -2.3333333333333335f));
+    return r;
+}
+__device__ __forceinline__ double pow_m73(double h) { return 1.0 / (h * h * cbrt(h)); }
 __device__ __forceinline__ float  real_sqrt(float a)  { return sqrtf(a); }
 __device__ __forceinline__ double real_sqrt(double a) { return sqrt(a); }
-__device__ __forceinline__ float  real_exp(float a)  { return __expf(a); }
-__device__ __forceinline__ double real_exp(double a) { return exp(a); }
-// h^(7/3) for the Manning term
-__device__ __forceinline__ float  pow73(float h)  { return h * h * cbrtf(h); }
-__device__ __forceinline__ double pow73(double h) { return h * h * cbrt(h); }
 
 __device__ __forceinline__ void atomic_max_lambda(Ctl *ctl, double lam)
 {

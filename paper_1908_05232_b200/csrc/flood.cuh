@@ -40,26 +40,26 @@ struct FloodArgs {
 template <typename T>
 __device__ __forceinline__ void riemann(T g, T hL, T uL, T vL, T hR, T uR, T vR, T &f0, T &f1, T &f2)
 {
-    const T cL = real_sqrt(g * hL), cR = real_sqrt(g * hR);
-    T sL, sR;
-    if (hL <= T(0)) { sL = uR - T(2) * cR; sR = uR + cR; }
-    else if (hR <= T(0)) { sL = uL - cL; sR = uL + T(2) * cL; }
-    else {
-        const T us = T(0.5) * (uL + uR) + cL - cR;
-        const T cs = T(0.5) * (cL + cR) + T(0.25) * (uL - uR);
-        sL = fmin(uL - cL, us - cs);
-        sR = fmax(uR + cR, us + cs);
-    }
+    // branch-free: selects for the dry-bed speeds, and the upwind cases fall out of clamping the
+    // wave speeds (s_L <- min(s_L,0), s_R <- max(s_R,0)): w = 0 gives F_L, w = 1 gives F_R.
+    const T cL = fast_sqrt(g * hL), cR = fast_sqrt(g * hR);
+    const T us = T(0.5) * (uL + uR) + cL - cR;
+    const T cs = T(0.5) * (cL + cR) + T(0.25) * (uL - uR);
+    T sL = fmin(uL - cL, us - cs);
+    T sR = fmax(uR + cR, us + cs);
+    const bool dryL = hL <= T(0), dryR = hR <= T(0);
+    sL = dryL ? uR - T(2) * cR : sL;  sR = dryL ? uR + cR : sR;
+    sR = dryR ? uL + T(2) * cL : sR;  sL = dryR ? uL - cL : sL;
+    sL = fmin(sL, T(0)); sR = fmax(sR, T(0));
     const T qL = hL * uL, qR = hR * uR;
     const T pL = qL * uL + T(0.5) * g * hL * hL;
     const T pR = qR * uR + T(0.5) * g * hR * hR;
-    if (sL >= T(0)) { f0 = qL; f1 = pL; }
-    else if (sR <= T(0)) { f0 = qR; f1 = pR; }
-    else {
-        const T inv = fast_rcp(sR - sL), ss = sL * sR;
-        f0 = (sR * qL - sL * qR + ss * (hR - hL)) * inv;
-        f1 = (sR * pL - sL * pR + ss * (qR - qL)) * inv;
-    }
+    // HLL written around F_L: F = F_L + w [(F_R - F_L) - s_R (U_R - U_L)], w = -s_L/(s_R - s_L).
+    // Equal states give F_L exactly whatever the rounding of w (lake at rest stays at rest).
+    const T w = -sL * fast_rcp(fmax(sR - sL, T(1e-30)));      // s_R = s_L = 0 only if s_L = 0: w = 0
+    const T dq = qR - qL;
+    f0 = qL + w * (dq - sR * (hR - hL));
+    f1 = pL + w * ((pR - pL) - sR * dq);
     f2 = f0 * (f0 >= T(0) ? vL : vR);
 }
 
@@ -109,10 +109,10 @@ __device__ __forceinline__ void finish_cell(const FloodArgs<T> &a, T dt, T h, T 
     lam = T(0);
     if (hn > a.h_dry) {
         const T n = a.couple ? n0 * (T(1) + T(min(np, a.n_cap))) : n0;
-        const T D = T(1) + dt * a.g * n * n * real_sqrt(qxn * qxn + qyn * qyn) / pow73(hn);
+        const T D = T(1) + dt * a.g * n * n * fast_sqrt(qxn * qxn + qyn * qyn) * pow_m73(hn);
         const T rD = fast_rcp(D);
         qxn *= rD; qyn *= rD;
-        const T rh = fast_rcp(hn), c = real_sqrt(a.g * hn);
+        const T rh = fast_rcp(hn), c = fast_sqrt(a.g * hn);
         lam = fmax((fabs(qxn * rh) + c) * a.inv_dx, (fabs(qyn * rh) + c) * a.inv_dy);
     } else { qxn = T(0); qyn = T(0); }
 }
@@ -205,7 +205,7 @@ struct TileSmem {
 };
 
 template <typename T>
-__global__ void __launch_bounds__(FLOOD_TILE_THREADS) flood_tile_kernel(FloodArgs<T> a)
+__global__ void __launch_bounds__(FLOOD_TILE_THREADS, sizeof(T) == 4 ? 3 : 1) flood_tile_kernel(FloodArgs<T> a)
 {
     extern __shared__ __align__(32) unsigned char smem_raw[];
     TileSmem<T> &s = *reinterpret_cast<TileSmem<T> *>(smem_raw);

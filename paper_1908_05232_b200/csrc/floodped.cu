@@ -167,7 +167,7 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
     for (int k = 0; k < 3; ++k) a.hr_edge[k] = (T)p.hr_edges[k];
     for (int k = 0; k < 4; ++k) a.speed_wet[k] = (T)p.speed_wet[k];
     a.inv_tau = (T)(1.0 / p.tau); a.A_s = (T)p.A_s; a.inv_B = (T)(1.0 / p.B_s); a.two_r = (T)(2.0 * p.radius);
-    a.R_int = (T)p.R_int; a.vmax_factor = (T)p.vmax_factor; a.t_pick = (T)p.t_pick; a.t_drop = (T)p.t_drop;
+    a.R_int = (T)p.R_int; a.R2 = (T)(p.R_int * p.R_int); a.vmax_factor = (T)p.vmax_factor; a.t_pick = (T)p.t_pick; a.t_drop = (T)p.t_drop;
     a.n_targets = p.n_targets; a.exit_target = p.exit_target; a.storage_target = p.storage_target;
     a.drop_target = p.drop_target;
     a.storage_i = p.storage_cell % s->grid.nx; a.storage_j = p.storage_cell / s->grid.nx;

@@ -25,7 +25,7 @@ struct PedArgs {
     int nx, ny, kbin, nbx, nby, nbins;
     T inv_dx, inv_dy, dxk;
     T h_dry, hr_edge[3], speed_wet[4];
-    T inv_tau, A_s, inv_B, two_r, R_int, vmax_factor, t_pick, t_drop;
+    T inv_tau, A_s, inv_B, two_r, R_int, R2, vmax_factor, t_pick, t_drop;
     int n_targets, exit_target, storage_target, drop_target;
     int n_exit; int exit_i[16], exit_j[16];
     int storage_i, storage_j, drop_i, drop_j, arrive;
@@ -197,21 +197,28 @@ __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
     const int ix = c % a.nx, iy = c / a.nx;
     const int bx = ix / a.kbin, by = iy / a.kbin;
 
-    // 4. social repulsion over the 3 x 3 adjacent bins (C24, C26) + N_p of my cell
+    // 4. social repulsion over the 3 x 3 adjacent bins (C24, C26): three contiguous
+    //    index ranges, one per bin row
     T ax = T(0), ay = T(0);
-    int same = 0, lower = 0;
     for (int jy = max(by - 1, 0); jy <= min(by + 1, a.nby - 1); ++jy) {
         const int s0 = a.start[jy * a.nbx + max(bx - 1, 0)];
         const int s1 = a.start[jy * a.nbx + min(bx + 1, a.nbx - 1) + 1];
         for (int j = s0; j < s1; ++j) {
             const T ddx = x - B.x[j], ddy = y - B.y[j];
-            const T dist = real_sqrt(ddx * ddx + ddy * ddy);
-            if (dist > T(0) && dist < a.R_int) {
-                const T f = a.A_s * real_exp((a.two_r - dist) * a.inv_B) / dist;
+            const T d2 = ddx * ddx + ddy * ddy;
+            if (d2 > T(0) && d2 < a.R2) {
+                const T rinv = fast_rsqrt(d2);
+                const T f = a.A_s * fast_exp((a.two_r - d2 * rinv) * a.inv_B) * rinv;
                 ax += f * ddx; ay += f * ddy;
             }
-            if (jy == by && B.cell[j] == c) { same += 1; lower += (j < d); }
         }
+    }
+    // N_p of my cell: agents of my own bin that share my cell
+    int same = 0, lower = 0;
+    {
+        const int b = by * a.nbx + bx;
+        for (int j = a.start[b]; j < a.start[b + 1]; ++j)
+            if (B.cell[j] == c) { same += 1; lower += (j < d); }
     }
     // (O) one agent per occupied cell publishes N_p; remember the cell for next step's clear
     if (lower == 0) a.occ[c] = (uint8_t)min(same, 255);
