@@ -150,7 +150,9 @@ def run_ours(args):
     real = np.float32 if sc.real_bits == 32 else np.float64
     ncell, npeds = sc.nx * sc.ny, sc.n_peds
     g = binding.Sim(sc, device=f"cuda:{local}")
-    g.set_flood_variant(args.flood_variant if sc.nx % 4 == 0 else 0)
+    if args.flood_variant >= 0:
+        g.set_flood_variant(args.flood_variant)
+    variant = g.flood_variant()
     kps = g.kernels_per_step()
 
     def barrier():
@@ -252,14 +254,14 @@ def run_ours(args):
         "config": {"workload": f"config{args.config}: {sc.name}", "nx": sc.nx, "ny": sc.ny, "dx": sc.dx,
                    "pedestrians": npeds, "active_pedestrians": active,
                    "l2_policy": "inputs larger than L2 (no flush)" if ncell * fb > 126e6 else "working set fits L2: latency-bound config, roofline not meaningful",
-                   "flood_variant": args.flood_variant, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+                   "flood_variant": variant, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": world * ncell * e2e_done / e2e_s, "unit": "cell-updates/s",
                 "h2d_bytes_per_step": h2d / e2e_done, "d2h_bytes_per_step": d2h / e2e_done,
                 "steps": e2e_done, "seconds": e2e_s,
                 "what": "sim_write_flood+sim_write_peds from pinned host, sim_step, sim_read_conserved+sim_read_peds+sim_get_stats to host"},
         "gpu_launches": int(done * kps),
-        "roofline": {"bound": "hbm", "kernel": "flood_tile_kernel<float>" if args.flood_variant else "flood_cell_kernel<float>",
+        "roofline": {"bound": "hbm", "kernel": ("flood_cell_kernel", "flood_tile_kernel", "flood_march_kernel")[variant] + ("<float>" if sc.real_bits == 32 else "<double>"),
                      "achieved": flood_gbs, "peak": peak, "unit": "GB/s", "frac": flood_gbs / peak,
                      "peak_source": peak_src, "frac_of_8TBs_spec": flood_gbs / 8000.0,
                      "bytes_per_cell": fb, "kernel_ms": flood_ms, "traffic": None,
@@ -283,7 +285,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--flood-variant", type=int, default=1, choices=[0, 1])
+    ap.add_argument("--flood-variant", type=int, default=-1, choices=[-1, 0, 1, 2], help="-1: the library default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -176,9 +176,11 @@ int sim_write_peds(sim_t *s, const void *x, const void *y, const void *vx, const
                    const uint8_t *fsm, const uint8_t *active, const void *timer);
 int sim_set_time(sim_t *s, double t, double dt);
 int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete);
-/* Choose the flood kernel: 0 = reference-shaped (one thread per cell, 4 faces each),
- * 1 = tiled (each face once, shared-memory staging).  Default 1. */
+/* Choose the flood kernel: 0 = one thread per cell, 4 faces each (any nx); 1 = 64x16 tiles, each
+ * face once, shared-memory staging (nx % 4 == 0); 2 = row-marching strips of 256 columns, each
+ * face once, rows prefetched in registers (any nx).  Default: 2 from 2^22 cells, else 1 (or 0). */
 int sim_set_flood_variant(sim_t *s, int32_t variant);
+int sim_get_flood_variant(const sim_t *s);         /* the kernel in use, or SIM_EINVAL */
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
 

@@ -19,7 +19,7 @@ SIM_OK, SIM_EINVAL, SIM_ENOMEM, SIM_ECUDA, SIM_ENOTFINITE = 0, -1, -2, -3, -4
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
-    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_set_flood_variant",
+    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_set_flood_variant", "sim_get_flood_variant",
     "sim_kernels_per_step", "sim_last_error", "sim_destroy",
 ]
 
@@ -109,6 +109,7 @@ def load_library(path: str = LIB_PATH):
     L.sim_set_time.argtypes = [_vp, C.c_double, C.c_double]
     L.sim_set_barrier.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32]
     L.sim_set_flood_variant.argtypes = [_vp, C.c_int32]
+    L.sim_get_flood_variant.argtypes = [_vp]
     L.sim_kernels_per_step.argtypes = [_vp]
     L.sim_last_error.argtypes = [_vp]
     L.sim_last_error.restype = C.c_char_p
@@ -202,6 +203,7 @@ class Sim:
         torch.cuda.set_device(self.device)
         self.real = np.float64 if sc.real_bits == 64 else np.float32
         self.nx, self.ny, self.ncell, self.n_peds = sc.nx, sc.ny, sc.nx * sc.ny, int(sc.px.shape[0])
+        self.dx, self.dy = float(sc.dx), float(sc.dy)
         m = _Marshalled(sc)
         self._ws = None
         ws_ptr = None
@@ -250,6 +252,9 @@ class Sim:
 
     def set_flood_variant(self, v):
         self._chk(self._L.sim_set_flood_variant(self._h, int(v)))
+
+    def flood_variant(self) -> int:
+        return self._L.sim_get_flood_variant(self._h)
 
     # -- read-back (host numpy)
     def read_flood(self, fields=("h", "u", "v", "z", "hr")):

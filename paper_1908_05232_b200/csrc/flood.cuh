@@ -30,6 +30,8 @@ struct FloodArgs {
     const T *n0;                      // initial Manning n_M per cell
     const uint8_t *occ;               // N_p per cell of the current step (saturated at 255)
     const uint8_t *inflow[4];         // per edge cell: number of inflow faces on that side (W,E,S,N)
+    const uint8_t *chunk_flag;        // march kernel: 1 = chunk takes the general path (flood_march.cuh)
+    int R;                            // march kernel: rows per chunk
     Ctl *ctl;
 };
 

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "flood.cuh"
+#include "flood_march.cuh"
 #include "peds.cuh"
 
 using namespace fp;
@@ -56,6 +57,8 @@ struct sim {
     double *stat_d = nullptr;       // [4] volume, max_h, max_hr, n_bad ; [4] ped bad
     unsigned long long *stat_hist = nullptr;   // [6]
     int flood_variant = 1;
+    int march_R = 64, march_gx = 1, march_gy = 1;
+    uint8_t *chunk_flag = nullptr;
     int exit_i[16]{}, exit_j[16]{};
     cudaGraphExec_t graph1 = nullptr, graphN = nullptr;
     std::string err;
@@ -107,6 +110,7 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 2; ++k) s->ped_out_i32[k] = b.take<int32_t>(np);
     s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(np);
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
+    s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * s->march_gy);
     s->scan_status = b.take<unsigned long long>((size_t)(s->nbins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1);
     return (b.off + 255) & ~size_t(255);
 }
@@ -128,6 +132,12 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     s->kbin = (int)std::ceil(p->R_int / dmin); if (s->kbin < 1) s->kbin = 1;     // C26
     s->nbx = (g->nx + s->kbin - 1) / s->kbin; s->nby = (g->ny + s->kbin - 1) / s->kbin;
     s->nbins = s->nbx * s->nby;
+    // march kernel geometry: strips of MW columns, chunks of R rows; R shrinks until the grid
+    // fills the 148 SMs a few times over
+    s->march_gx = (g->nx + MW - 1) / MW;
+    s->march_R = 64;
+    while (s->march_R > 16 && (long long)s->march_gx * ((g->ny + s->march_R - 1) / s->march_R) < 148 * 4) s->march_R /= 2;
+    s->march_gy = (g->ny + s->march_R - 1) / s->march_R;
     s->n_inflow = p->n_inflow_faces; s->n_hydro = p->n_hydro; s->n_line = p->n_line; s->n_targets = p->n_targets;
     return SIM_OK;
 }
@@ -142,6 +152,7 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     for (int k = 0; k < 2; ++k) { a.h[k] = (T *)s->h[k]; a.qx[k] = (T *)s->qx[k]; a.qy[k] = (T *)s->qy[k]; }
     a.zs = (const T *)s->zs; a.n0 = (const T *)s->n0; a.occ = s->occ;
     for (int k = 0; k < 4; ++k) a.inflow[k] = s->inflow[k];
+    a.chunk_flag = s->chunk_flag; a.R = s->march_R;
     a.ctl = s->ctl;
     return a;
 }
@@ -215,7 +226,9 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
     } else k = 4;
     FloodArgs<T> fa = flood_args<T>(s);
     mark();
-    if (s->flood_variant == 1) {
+    if (s->flood_variant == 2) {
+        flood_march_kernel<T><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
+    } else if (s->flood_variant == 1) {
         dim3 grid((s->grid.nx + TX - 1) / TX, (s->grid.ny + TY - 1) / TY);
         flood_tile_kernel<T><<<grid, FLOOD_TILE_THREADS, sizeof(TileSmem<T>), st>>>(fa);
     } else {
@@ -285,6 +298,7 @@ template <typename T> int build_graphs(sim *s)
 
 template <typename T> int refresh_dt(sim *s)      // lambda of the state in place -> dt, q_in, halt
 {
+    flood_chunk_flags_kernel<T><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const T *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
     flood_lambda_kernel<T><<<592, 256, 0, s->stream>>>(flood_args<T>(s));
     tail_kernel<T><<<1, 32, 0, s->stream>>>(tail_args<T>(s), 1);
     CU(cudaGetLastError());
@@ -459,7 +473,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         const double dmin = grid->dx < grid->dy ? grid->dx : grid->dy;
         s->prm.dt_max = grid->real_bits == 64 ? default_dt_max<double>(peds, p, dmin) : default_dt_max<float>(peds, p, dmin);
     }
-    s->flood_variant = (nx % 4 == 0) ? 1 : 0;
+    s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? 2 : (nx % 4 == 0) ? 1 : 0;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -525,10 +539,12 @@ extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
 
 extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? 6 : 2) : 0; }
 
+extern "C" int sim_get_flood_variant(const sim_t *s) { return s ? s->flood_variant : SIM_EINVAL; }
+
 extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
 {
     if (!s) return SIM_EINVAL;
-    if (variant != 0 && variant != 1) return fail(s, SIM_EINVAL, "variant must be 0 or 1");
+    if (variant < 0 || variant > 2) return fail(s, SIM_EINVAL, "variant must be 0, 1 or 2");
     if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");
     CU(cudaStreamSynchronize(s->stream));
     s->flood_variant = variant;

@@ -23,7 +23,12 @@ def _compare_flood(o, g, bits):
     sa, sb = g.stats(), o.stats()
     assert abs(sa["dt"] - sb["dt"]) <= 10 * TOL[bits] * sb["dt"]
     assert abs(sa["t"] - sb["t"]) <= 1e-12 * max(sb["t"], 1.0)
-    assert sa["neg_depth_clamps"] == sb["neg_depth_clamps"]
+    # C12 clamp: a depth within rounding of zero may be clamped on one side only, so the COUNT can
+    # differ by such cells, but each of them holds less than tol * max h, hence so does the volume
+    dn = abs(sa["neg_depth_clamps"] - sb["neg_depth_clamps"])
+    hmax = max(float(np.max(b["h"])), 1e-300)
+    assert abs(sa["clamped_volume"] - sb["clamped_volume"]) <= TOL[bits] * hmax * g.dx * g.dy * max(dn, 1)
+    assert dn <= 2
 
 
 def _ped_compare(o, g, sc, p_before, dt, dep_before=(0, 0)):
@@ -82,20 +87,20 @@ def _one_step(sc, evolve, variant=None, check_peds=True):
 
 # ------------------------------------------------------------------ flood, single step
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("evolve", [0, 7, 40])
 def test_config1_single_step_fp64(variant, evolve):
     _one_step(S.make(1), evolve, variant)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_config2_single_step_fp32_wet_dry_inflow(variant):
     sc = S.make(2)
     sc.hydro_q = sc.hydro_q * 20.0            # a stronger flood so that a lot of the hall is wet
     _one_step(sc, 300, variant)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_config4_mini_single_step_fp32_buildings_all_hr_classes(variant):
     sc = S.make(4, n=256, n_peds=5000)
     o, g = _one_step(sc, 150, variant)
@@ -103,7 +108,7 @@ def test_config4_mini_single_step_fp32_buildings_all_hr_classes(variant):
     assert hist[1] > 0 and hist[2] > 0 and hist[3] > 0      # low, medium, high all present
 
 
-@pytest.mark.parametrize("nx,ny", [(4, 4), (64, 16), (100, 37), (130, 50), (33, 9), (7, 5)])
+@pytest.mark.parametrize("nx,ny", [(4, 4), (64, 16), (100, 37), (130, 50), (33, 9), (7, 5), (300, 70), (257, 33), (512, 130)])
 def test_ragged_tiles_and_tiny_grids(nx, ny):
     rng = np.random.default_rng(nx * 100 + ny)
     z = 0.2 * rng.random((ny, nx))
@@ -112,7 +117,7 @@ def test_ragged_tiles_and_tiny_grids(nx, ny):
     for bits in (64, 32):
         sc = box(nx, ny, dx=0.5, real_bits=bits, z=z, h0=h0, u0=rng.normal(0, 0.5, (ny, nx)),
                  v0=rng.normal(0, 0.5, (ny, nx)), mask=mask, manning=0.03, dt_max=0.05)
-        for variant in ((0, 1) if nx % 4 == 0 else (0,)):
+        for variant in ((0, 1, 2) if nx % 4 == 0 else (0, 2)):
             o, g = make_pair(sc, evolve=0, variant=variant)
             sync(o, g, sc)
             for _ in range(3):
@@ -120,6 +125,42 @@ def test_ragged_tiles_and_tiny_grids(nx, ny):
                 # re-sync so that each step starts from identical inputs
                 _compare_flood(o, g, bits)
                 sync(o, g, sc)
+
+
+@pytest.mark.parametrize("bits", [32, 64])
+@pytest.mark.parametrize("solids", [False, True])
+def test_march_kernel_interior_chunks_take_the_fast_path(bits, solids):
+    """1024 x 100 cells: 4 strips of 256 columns and chunks of 16 rows, so the two middle strips
+    hold chunks that touch neither the domain edge nor (without solids) a solid cell; with solids a
+    few isolated solid cells land inside and on the halo of such chunks.  Wet/dry mix over a rough
+    bed, inflow on the west edge; three steps, each from identical state."""
+    nx, ny = 1024, 100
+    rng = np.random.default_rng(7 + bits + solids)
+    jj, ii = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    z = 0.3 * (1 + np.sin(ii / 37.0) * np.cos(jj / 11.0)) + 0.02 * rng.random((ny, nx))
+    h0 = np.maximum(0.0, 0.35 - z) + np.where(rng.random((ny, nx)) < 0.05, 0.3 * rng.random((ny, nx)), 0.0)
+    mask = np.zeros((ny, nx), np.uint8)
+    if solids:
+        for (i, j) in [(255, 40), (256, 41), (511, 47), (512, 48), (600, 31), (600, 32), (700, 63), (300, 16), (301, 15)]:
+            mask[j, i] = 1
+        mask[50:60, 400:420] = 1
+    sc = box(nx, ny, dx=0.25, real_bits=bits, z=z, h0=h0, u0=rng.normal(0, 0.3, (ny, nx)),
+             v0=rng.normal(0, 0.3, (ny, nx)), mask=mask, manning=0.02, dt_max=0.02,
+             inflow_cell=np.arange(10, 30, dtype=np.int32) * nx, inflow_side=np.zeros(20, np.uint8),
+             hydro_t=np.array([0.0, 1.0]), hydro_q=np.array([3.0, 3.0]))
+    o, g = make_pair(sc, evolve=0, variant=2)
+    sync(o, g, sc)
+    for _ in range(3):
+        o.step(1); g.step(1)
+        _compare_flood(o, g, bits)
+        sync(o, g, sc)
+    # and the three kernels agree with one another after a few free-running steps
+    outs = []
+    for variant in (0, 1, 2):
+        g2 = binding.Sim(sc); g2.set_flood_variant(variant); g2.step(5)
+        outs.append(g2.read_conserved())
+    for k in ("h", "qx", "qy"):
+        assert mixed(outs[1][k], outs[0][k]) <= 20 * TOL[bits] and mixed(outs[2][k], outs[0][k]) <= 20 * TOL[bits]
 
 
 def test_tiled_kernel_rejects_unaligned_width():
@@ -253,7 +294,7 @@ def test_t_end_lands_and_halts_on_device():
 def test_no_pedestrians_and_lake_at_rest_on_gpu():
     sc = S.make(1, n_peds=0)
     sc.h0 = np.maximum(0.0, 0.2 - sc.z)                 # island
-    for variant in (0, 1):
+    for variant in (0, 1, 2):
         g = binding.Sim(sc); g.set_flood_variant(variant)
         g.step(500)
         c = g.read_conserved()
