@@ -28,7 +28,9 @@ def _compare_flood(o, g, bits):
     dn = abs(sa["neg_depth_clamps"] - sb["neg_depth_clamps"])
     hmax = max(float(np.max(b["h"])), 1e-300)
     assert abs(sa["clamped_volume"] - sb["clamped_volume"]) <= TOL[bits] * hmax * g.dx * g.dy * max(dn, 1)
-    assert dn <= 2
+    # a cell clamped on one side only ends with a depth in (0, tol * max h] on the other side
+    near = int(np.sum((b["h"] > 0) & (b["h"] <= TOL[bits] * hmax))) + int(np.sum((a["h"] > 0) & (a["h"] <= TOL[bits] * hmax)))
+    assert dn <= max(2, near), (dn, near)
 
 
 def _ped_compare(o, g, sc, p_before, dt, dep_before=(0, 0)):
