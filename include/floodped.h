@@ -178,7 +178,8 @@ int sim_set_time(sim_t *s, double t, double dt);
 int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete);
 /* Choose the flood kernel: 0 = one thread per cell, 4 faces each (any nx); 1 = 64x16 tiles, each
  * face once, shared-memory staging (nx % 4 == 0); 2 = row-marching strips of 256 columns, each
- * face once, rows prefetched in registers (any nx).  Default: 2 from 2^22 cells, else 1 (or 0). */
+ * face once, rows prefetched in registers (any nx); 3 = as 2 with two columns per thread and
+ * 64/128-bit accesses (nx % 2 == 0).  Default: 3 (else 2) from 2^22 cells, else 1 (or 0). */
 int sim_set_flood_variant(sim_t *s, int32_t variant);
 int sim_get_flood_variant(const sim_t *s);         /* the kernel in use, or SIM_EINVAL */
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */

@@ -1,0 +1,246 @@
+// flood_tmarch.cuh -- variant 6/7 of step (F)+(T): the row-marching flood-cell update of
+// flood_march2.cuh (Eq. (2); same face_eta(), finish_hat2(), same strip/chunk geometry and
+// shared-memory exchange) with the rows of an interior chunk brought in by the TMA engine.
+//
+//   Why: ncu of variant 3 (two columns per thread, 117 registers, 16 warps/SM) shows the fewest
+//   instructions per cell of all variants (195) but IPC 0.52 with long-scoreboard (global-load
+//   latency) as the dominant stall: register prefetch two rows ahead does not keep enough bytes in
+//   flight at that occupancy.  Here one elected thread issues, per row, six 1-D bulk copies
+//   (cp.async.bulk global -> shared: h, qx, qy, z, n0 of the strip's 256 columns and their N_p
+//   bytes) into a ring of STAGES row buffers, each completing on an mbarrier; the ring runs STAGES
+//   rows ahead of the arithmetic at no register cost.  The slot read in iteration r is refilled
+//   with row r+STAGES right after that iteration's __syncthreads (every thread has its values in
+//   registers by then).
+//
+//   Chunks that touch the domain edge or a solid cell (chunk_flag = 1) take march2_chunk<GEN=true>
+//   with plain loads.  Needs nx % 16 == 0 (16-byte alignment of every row segment).
+#pragma once
+
+#include "flood_march2.cuh"
+
+namespace fp {
+
+template <typename T>
+struct __align__(16) RowStage {
+    T h[MW], qx[MW], qy[MW], z[MW], n0[MW];
+    uint8_t occ[MW];
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// one row segment (columns x0 .. x0+MW-1 of row j) -> stage
+template <typename T>
+__device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, const T *QX, const T *QY,
+                                             RowStage<T> &st, uint64_t *bar, int x0, int j)
+{
+    const size_t c = (size_t)j * a.nx + x0;
+    constexpr uint32_t RB = MW * sizeof(T);
+    mbar_expect_tx(bar, 5 * RB + MW);
+    bulk_g2s(st.h, H + c, RB, bar);
+    bulk_g2s(st.qx, QX + c, RB, bar);
+    bulk_g2s(st.qy, QY + c, RB, bar);
+    bulk_g2s(st.z, a.zs + c, RB, bar);
+    bulk_g2s(st.n0, a.n0 + c, RB, bar);
+    bulk_g2s(st.occ, a.occ + c, MW, bar);
+}
+
+// interior chunk (no domain edge, no solid cell in it or in its halo): rows y0-1 .. y0+R all exist
+template <typename T, int CPT, int STAGES>
+__device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, CPT> &s, RowStage<T> *ring,
+                                          uint64_t *bars, int x0, int y0, int R)
+{
+    constexpr int NT = MW / CPT;
+    const int tid = threadIdx.x;
+    const int nx = a.nx;
+    const int p = a.ctl->parity;
+    const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
+    const T *__restrict__ Z = a.zs;
+    T *__restrict__ Ho = a.h[p ^ 1], *__restrict__ QXo = a.qx[p ^ 1], *__restrict__ QYo = a.qy[p ^ 1];
+    const T dt = (T)a.ctl->dt;
+    const T dtdx = dt * a.inv_dx, dtdy = dt * a.inv_dy;
+    const T g = a.g, h_dry = a.h_dry;
+    const int i = x0 + tid * CPT;
+    const int y1 = y0 + R;
+    const int nrows = R + 2;                           // ring row r holds grid row y0 - 1 + r
+
+    if (tid == 0) {
+        for (int k = 0; k < STAGES; ++k) mbar_init(&bars[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0)
+        for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row(a, H, QX, QY, ring[r], &bars[r], x0, y0 - 1 + r);
+
+    // ---- pre-pass: strip-edge data for every row of the chunk (as in variants 2, 3)
+    for (int k = tid; k < R; k += NT) {
+        const int j = y0 + k;
+        Raw4<T> l = march_load<T, false>(H, QX, QY, Z, x0 + MW - 1, j, nx, a.ny);
+        Raw4<T> r = march_load<T, false>(H, QX, QY, Z, x0 + MW, j, nx, a.ny);
+        Raw4<T> w = march_load<T, false>(H, QX, QY, Z, x0 - 1, j, nx, a.ny);
+        T el, ul, vl, er_, ur, vr, ew, uw, vw, f0, f1L, f1R, f2;
+        march_prims<T, false>(l, h_dry, el, ul, vl);
+        march_prims<T, false>(r, h_dry, er_, ur, vr);
+        march_prims<T, false>(w, h_dry, ew, uw, vw);
+        face_eta<T, false, false>(g, el, ul, vl, l.z, er_, ur, vr, r.z, f0, f1L, f1R, f2);
+        s.er[0][k] = f0; s.er[1][k] = f1L; s.er[2][k] = f2;
+        s.sw[0][k] = ew; s.sw[1][k] = uw; s.sw[2][k] = vw; s.sw[3][k] = w.z;
+    }
+
+    // halo row y0-1 (ring row 0) becomes "prev"
+    T eta_p[CPT], u_p[CPT], v_p[CPT], z_p[CPT];
+    {
+        mbar_wait(&bars[0], 0);
+        const RowStage<T> &st = ring[0];
+        const VecN<T, CPT> h = *reinterpret_cast<const VecN<T, CPT> *>(&st.h[tid * CPT]);
+        const VecN<T, CPT> qx = *reinterpret_cast<const VecN<T, CPT> *>(&st.qx[tid * CPT]);
+        const VecN<T, CPT> qy = *reinterpret_cast<const VecN<T, CPT> *>(&st.qy[tid * CPT]);
+        const VecN<T, CPT> z = *reinterpret_cast<const VecN<T, CPT> *>(&st.z[tid * CPT]);
+#pragma unroll
+        for (int k = 0; k < CPT; ++k) {
+            Raw4<T> q{h.v[k], qx.v[k], qy.v[k], z.v[k]};
+            march_prims<T, false>(q, h_dry, eta_p[k], u_p[k], v_p[k]);
+            z_p[k] = q.z;
+        }
+    }
+    __syncthreads();                                   // slot 0 consumed; er/sw visible
+    if (tid == 0 && STAGES < nrows) tm_issue_row(a, H, QX, QY, ring[0], &bars[0], x0, y0 - 1 + STAGES);
+
+    T ah[CPT], ax[CPT], ay[CPT], n0_p[CPT];
+    int occ_p[CPT];
+#pragma unroll
+    for (int k = 0; k < CPT; ++k) { ah[k] = ax[k] = ay[k] = n0_p[k] = T(0); occ_p[k] = 0; }
+    T lam = T(0), clamp_h = T(0);
+    int clamp_n = 0;
+    int slot = 1 % STAGES;
+    uint32_t phase = (1 / STAGES) & 1;
+
+#pragma unroll 2
+    for (int jj = y0; jj <= y1; ++jj) {
+        const int r = jj - y0 + 1;
+        mbar_wait(&bars[slot], phase);
+        const RowStage<T> &st = ring[slot];
+        const VecN<T, CPT> hv = *reinterpret_cast<const VecN<T, CPT> *>(&st.h[tid * CPT]);
+        const VecN<T, CPT> qxv = *reinterpret_cast<const VecN<T, CPT> *>(&st.qx[tid * CPT]);
+        const VecN<T, CPT> qyv = *reinterpret_cast<const VecN<T, CPT> *>(&st.qy[tid * CPT]);
+        const VecN<T, CPT> zv = *reinterpret_cast<const VecN<T, CPT> *>(&st.z[tid * CPT]);
+        const VecN<T, CPT> n0_c = *reinterpret_cast<const VecN<T, CPT> *>(&st.n0[tid * CPT]);
+        const ByteN<CPT> occ_c = *reinterpret_cast<const ByteN<CPT> *>(&st.occ[tid * CPT]);
+        T eta[CPT], u[CPT], v[CPT], z[CPT], hc[CPT], qxc[CPT], qyc[CPT];
+#pragma unroll
+        for (int k = 0; k < CPT; ++k) {
+            Raw4<T> q{hv.v[k], qxv.v[k], qyv.v[k], zv.v[k]};
+            march_prims<T, false>(q, h_dry, eta[k], u[k], v[k]);
+            z[k] = q.z; hc[k] = q.h; qxc[k] = q.qx; qyc[k] = q.qy;
+        }
+        const int b = jj & 1;
+        s.st[b][0][tid] = eta[CPT - 1]; s.st[b][1][tid] = u[CPT - 1];
+        s.st[b][2][tid] = v[CPT - 1];   s.st[b][3][tid] = z[CPT - 1];
+        __syncthreads();
+        if (tid == 0 && r + STAGES < nrows) tm_issue_row(a, H, QX, QY, ring[slot], &bars[slot], x0, y0 - 1 + r + STAGES);
+        if (++slot == STAGES) { slot = 0; phase ^= 1u; }
+
+        // south faces of the current row = north faces of the previous one (normal velocity v)
+        T g0[CPT], g1L[CPT], g1R[CPT], g2[CPT];
+#pragma unroll
+        for (int k = 0; k < CPT; ++k)
+            face_eta<T, false, true>(g, eta_p[k], v_p[k], u_p[k], z_p[k], eta[k], v[k], u[k], z[k], g0[k], g1L[k], g1R[k], g2[k]);
+
+        if (jj > y0) {                                 // finish row jj-1
+            const int j = jj - 1, bp = b ^ 1;
+            const T *fe = (tid == NT - 1) ? &s.er[0][j - y0] : &s.fx[bp][0][tid + 1];
+            const int stride = (tid == NT - 1) ? MARCH_MAX_R : NT;
+            VecN<T, CPT> ho, qxo, qyo;
+#pragma unroll
+            for (int k = 0; k < CPT; ++k) {
+                T hn = ah[k] - dtdy * g0[k], qxn = ax[k] - dtdy * g2[k], qyn = ay[k] - dtdy * g1L[k];
+                if (k == CPT - 1) { hn -= dtdx * fe[0]; qxn -= dtdx * fe[stride]; qyn -= dtdx * fe[2 * stride]; }
+                finish_hat2(a, dt, hn, qxn, qyn, n0_p[k], occ_p[k], lam, clamp_h, clamp_n);
+                ho.v[k] = hn; qxo.v[k] = qxn; qyo.v[k] = qyn;
+            }
+            const size_t c = (size_t)j * nx + i;
+            *reinterpret_cast<VecN<T, CPT> *>(Ho + c) = ho;
+            *reinterpret_cast<VecN<T, CPT> *>(QXo + c) = qxo;
+            *reinterpret_cast<VecN<T, CPT> *>(QYo + c) = qyo;
+        }
+        if (jj < y1) {                                 // enter row jj: west faces, start its accumulators
+            const T *sl = (tid == 0) ? &s.sw[0][jj - y0] : &s.st[b][0][tid - 1];
+            const int stride = (tid == 0) ? MARCH_MAX_R : NT;
+            T f0[CPT], f1L[CPT], f1R[CPT], f2[CPT];
+            face_eta<T, false, true>(g, sl[0], sl[stride], sl[2 * stride], sl[3 * stride], eta[0], u[0], v[0], z[0],
+                                     f0[0], f1L[0], f1R[0], f2[0]);
+#pragma unroll
+            for (int k = 1; k < CPT; ++k)
+                face_eta<T, false, true>(g, eta[k - 1], u[k - 1], v[k - 1], z[k - 1], eta[k], u[k], v[k], z[k],
+                                         f0[k], f1L[k], f1R[k], f2[k]);
+            s.fx[b][0][tid] = f0[0]; s.fx[b][1][tid] = f1L[0]; s.fx[b][2][tid] = f2[0];
+#pragma unroll
+            for (int k = 0; k < CPT; ++k) {
+                ah[k] = hc[k] + dtdx * f0[k] + dtdy * g0[k];
+                ax[k] = qxc[k] + dtdx * f1R[k] + dtdy * g2[k];
+                ay[k] = qyc[k] + dtdx * f2[k] + dtdy * g1R[k];
+                if (k < CPT - 1) { ah[k] -= dtdx * f0[k + 1]; ax[k] -= dtdx * f1L[k + 1]; ay[k] -= dtdx * f2[k + 1]; }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < CPT; ++k) {
+            eta_p[k] = eta[k]; u_p[k] = u[k]; v_p[k] = v[k]; z_p[k] = z[k];
+            n0_p[k] = n0_c.v[k]; occ_p[k] = a.couple ? (int)occ_c.v[k] : 0;
+        }
+    }
+    if (clamp_n) {
+        atomicAdd(&a.ctl->clamped_volume, (double)clamp_h * (double)a.cell_area);
+        atomicAdd(&a.ctl->neg_clamps, (unsigned long long)clamp_n);
+    }
+    return lam;
+}
+
+template <typename T, int STAGES> constexpr size_t tmarch_dyn_smem() { return sizeof(RowStage<T>) * STAGES + 8 * STAGES + 16; }
+
+template <typename T, int CPT, int STAGES>
+__global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? 4 : 2) flood_tmarch_kernel(FloodArgs<T> a)
+{
+    constexpr int NT = MW / CPT;
+    __shared__ March2Smem<T, CPT> s;
+    extern __shared__ __align__(16) unsigned char tm_dyn[];
+    if (a.ctl->halt) return;
+    RowStage<T> *ring = reinterpret_cast<RowStage<T> *>(tm_dyn);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(tm_dyn + sizeof(RowStage<T>) * STAGES);
+    const int x0 = blockIdx.x * MW, y0 = blockIdx.y * a.R;
+    const bool gen = a.chunk_flag[blockIdx.y * gridDim.x + blockIdx.x] != 0;
+    T lam = gen ? march2_chunk<T, CPT, true>(a, s, x0, y0, a.R)
+                : tmarch_chunk<T, CPT, STAGES>(a, s, ring, bars, x0, y0, a.R);
+    const int tid = threadIdx.x;
+    for (int o = 16; o > 0; o >>= 1) lam = fmax(lam, __shfl_xor_sync(0xffffffffu, lam, o));
+    __syncthreads();
+    if ((tid & 31) == 0) s.red[tid >> 5] = lam;
+    __syncthreads();
+    if (tid < 32) {
+        T m = tid < NT / 32 ? s.red[tid] : T(0);
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (tid == 0 && m > T(0)) atomic_max_lambda(a.ctl, (double)m);
+    }
+}
+
+}  // namespace fp

@@ -11,6 +11,9 @@
 
 #include "flood.cuh"
 #include "flood_march.cuh"
+#include "flood_march2.cuh"
+#include "flood_wmarch.cuh"
+#include "flood_tmarch.cuh"
 #include "peds.cuh"
 
 using namespace fp;
@@ -226,7 +229,26 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
     } else k = 4;
     FloodArgs<T> fa = flood_args<T>(s);
     mark();
-    if (s->flood_variant == 2) {
+    if (s->flood_variant == 6 || s->flood_variant == 7) {
+        if (s->flood_variant == 6) {
+            constexpr size_t dyn = tmarch_dyn_smem<T, 8>();
+            static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
+            (void)once;
+            flood_tmarch_kernel<T, 2, 8><<<dim3(s->march_gx, s->march_gy), MW / 2, dyn, st>>>(fa);
+        } else {
+            constexpr size_t dyn = tmarch_dyn_smem<T, 6>();
+            static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, 1, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
+            (void)once;
+            flood_tmarch_kernel<T, 1, 6><<<dim3(s->march_gx, s->march_gy), MW, dyn, st>>>(fa);
+        }
+    } else if (s->flood_variant == 5) {
+        static_assert(WM_MAX_R >= 64, "march_R is at most 64");
+        flood_wmarch_kernel<T><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
+    } else if (s->flood_variant == 4) {
+        flood_march2_kernel<T, 1><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
+    } else if (s->flood_variant == 3) {
+        flood_march2_kernel<T, 2><<<dim3(s->march_gx, s->march_gy), MW / 2, 0, st>>>(fa);
+    } else if (s->flood_variant == 2) {
         flood_march_kernel<T><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
     } else if (s->flood_variant == 1) {
         dim3 grid((s->grid.nx + TX - 1) / TX, (s->grid.ny + TY - 1) / TY);
@@ -473,7 +495,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         const double dmin = grid->dx < grid->dy ? grid->dx : grid->dy;
         s->prm.dt_max = grid->real_bits == 64 ? default_dt_max<double>(peds, p, dmin) : default_dt_max<float>(peds, p, dmin);
     }
-    s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? 2 : (nx % 4 == 0) ? 1 : 0;
+    s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? (nx % 2 == 0 ? 3 : 2) : (nx % 4 == 0) ? 1 : 0;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -544,7 +566,9 @@ extern "C" int sim_get_flood_variant(const sim_t *s) { return s ? s->flood_varia
 extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
 {
     if (!s) return SIM_EINVAL;
-    if (variant < 0 || variant > 2) return fail(s, SIM_EINVAL, "variant must be 0, 1 or 2");
+    if (variant < 0 || variant > 7) return fail(s, SIM_EINVAL, "variant must be 0..7");
+    if (variant >= 6 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
+    if (variant == 3 && s->grid.nx % 2 != 0) return fail(s, SIM_EINVAL, "the two-column march kernel needs nx % 2 == 0");
     if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");
     CU(cudaStreamSynchronize(s->stream));
     s->flood_variant = variant;
