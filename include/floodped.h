@@ -179,9 +179,13 @@ int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32
 /* Choose the flood kernel: 0 = one thread per cell, 4 faces each (any nx); 1 = 64x16 tiles, each
  * face once, shared-memory staging (nx % 4 == 0); 2 = row-marching strips of 256 columns, each
  * face once, rows prefetched in registers (any nx); 3 = as 2 with two columns per thread and
- * 64/128-bit accesses (nx % 2 == 0).  Default: 3 (else 2) from 2^22 cells, else 1 (or 0). */
+ * 64/128-bit accesses (nx % 2 == 0); 4 = as 3 with the rows of interior chunks brought in by TMA
+ * bulk copies into a shared-memory ring (nx % 16 == 0).
+ * Default: from 2^22 cells 4 (else 3, else 2), below that 1 (or 0). */
 int sim_set_flood_variant(sim_t *s, int32_t variant);
 int sim_get_flood_variant(const sim_t *s);         /* the kernel in use, or SIM_EINVAL */
+/* Rows per chunk of the row-marching kernels (8..64; default chosen by sim_create). Tuning hook. */
+int sim_set_march_rows(sim_t *s, int32_t rows);
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
 

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfloodped.so")
 SOURCES = ["floodped.cu"]
-HEADERS = ["common.cuh", "flood.cuh", "flood_march.cuh", "flood_march2.cuh", "flood_wmarch.cuh", "flood_tmarch.cuh", "peds.cuh", os.path.join("..", "..", "include", "floodped.h")]
+HEADERS = ["common.cuh", "flood.cuh", "flood_march.cuh", "flood_march2.cuh", "flood_tmarch.cuh", "peds.cuh", os.path.join("..", "..", "include", "floodped.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -25,7 +25,7 @@
 namespace fp {
 
 constexpr int MW = 256;               // columns per strip = threads per CTA
-constexpr int MARCH_MAX_R = 128;      // rows per chunk (runtime R <= this)
+constexpr int MARCH_MAX_R = 64;       // rows per chunk (runtime R <= this)
 
 template <typename T>
 struct MarchSmem {

@@ -1,5 +1,5 @@
 // flood_march2.cuh -- variant 3 of step (F)+(T): the row-marching flood-cell update of
-// flood_march.cuh (Eq. (2); same face flux face_eta() and same finish_hat()), with CPT
+// flood_march.cuh (Eq. (2); same face flux face_eta(); branch-free finish_hat2()), with CPT
 // adjacent columns per thread.
 //
 //   Why: ncu (profiles/r1_ncu_full_c5.md) shows variant 2 issue-bound (77 % of issue slots, about

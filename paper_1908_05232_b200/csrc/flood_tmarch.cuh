@@ -1,4 +1,4 @@
-// flood_tmarch.cuh -- variant 6/7 of step (F)+(T): the row-marching flood-cell update of
+// flood_tmarch.cuh -- variant 4 of step (F)+(T): the row-marching flood-cell update of
 // flood_march2.cuh (Eq. (2); same face_eta(), finish_hat2(), same strip/chunk geometry and
 // shared-memory exchange) with the rows of an interior chunk brought in by the TMA engine.
 //
@@ -218,8 +218,8 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
 
 template <typename T, int STAGES> constexpr size_t tmarch_dyn_smem() { return sizeof(RowStage<T>) * STAGES + 8 * STAGES + 16; }
 
-template <typename T, int CPT, int STAGES>
-__global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? 4 : 2) flood_tmarch_kernel(FloodArgs<T> a)
+template <typename T, int CPT, int STAGES, int MINB>
+__global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tmarch_kernel(FloodArgs<T> a)
 {
     constexpr int NT = MW / CPT;
     __shared__ March2Smem<T, CPT> s;

@@ -12,7 +12,6 @@
 #include "flood.cuh"
 #include "flood_march.cuh"
 #include "flood_march2.cuh"
-#include "flood_wmarch.cuh"
 #include "flood_tmarch.cuh"
 #include "peds.cuh"
 
@@ -113,7 +112,7 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 2; ++k) s->ped_out_i32[k] = b.take<int32_t>(np);
     s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(np);
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
-    s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * s->march_gy);
+    s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * ((s->grid.ny + 7) / 8));    // room for any R >= 8
     s->scan_status = b.take<unsigned long long>((size_t)(s->nbins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1);
     return (b.off + 255) & ~size_t(255);
 }
@@ -138,11 +137,22 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     // march kernel geometry: strips of MW columns, chunks of R rows; R shrinks until the grid
     // fills the 148 SMs a few times over
     s->march_gx = (g->nx + MW - 1) / MW;
-    s->march_R = 64;
-    while (s->march_R > 16 && (long long)s->march_gx * ((g->ny + s->march_R - 1) / s->march_R) < 148 * 4) s->march_R /= 2;
+    // about 12 waves of 148 SMs x 5 resident CTAs (measured best on 8192^2: R = 24..32)
+    s->march_R = (int)(((long long)g->ny * s->march_gx) / (12 * 148 * 5));
+    if (s->march_R > MARCH_MAX_R) s->march_R = MARCH_MAX_R;
+    if (s->march_R < 16) s->march_R = 16;
     s->march_gy = (g->ny + s->march_R - 1) / s->march_R;
     s->n_inflow = p->n_inflow_faces; s->n_hydro = p->n_hydro; s->n_line = p->n_line; s->n_targets = p->n_targets;
     return SIM_OK;
+}
+
+template <typename T, int CPT, int STAGES, int MINB>
+void launch_tmarch(const FloodArgs<T> &fa, dim3 grid, cudaStream_t st)
+{
+    constexpr size_t dyn = tmarch_dyn_smem<T, STAGES>();
+    static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, CPT, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
+    (void)once;
+    flood_tmarch_kernel<T, CPT, STAGES, MINB><<<grid, MW / CPT, dyn, st>>>(fa);
 }
 
 template <typename T> FloodArgs<T> flood_args(const sim *s)
@@ -229,23 +239,8 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
     } else k = 4;
     FloodArgs<T> fa = flood_args<T>(s);
     mark();
-    if (s->flood_variant == 6 || s->flood_variant == 7) {
-        if (s->flood_variant == 6) {
-            constexpr size_t dyn = tmarch_dyn_smem<T, 8>();
-            static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
-            (void)once;
-            flood_tmarch_kernel<T, 2, 8><<<dim3(s->march_gx, s->march_gy), MW / 2, dyn, st>>>(fa);
-        } else {
-            constexpr size_t dyn = tmarch_dyn_smem<T, 6>();
-            static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, 1, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
-            (void)once;
-            flood_tmarch_kernel<T, 1, 6><<<dim3(s->march_gx, s->march_gy), MW, dyn, st>>>(fa);
-        }
-    } else if (s->flood_variant == 5) {
-        static_assert(WM_MAX_R >= 64, "march_R is at most 64");
-        flood_wmarch_kernel<T><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
-    } else if (s->flood_variant == 4) {
-        flood_march2_kernel<T, 1><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
+    if (s->flood_variant == 4) {
+        launch_tmarch<T, 2, 5, 5>(fa, dim3(s->march_gx, s->march_gy), st);
     } else if (s->flood_variant == 3) {
         flood_march2_kernel<T, 2><<<dim3(s->march_gx, s->march_gy), MW / 2, 0, st>>>(fa);
     } else if (s->flood_variant == 2) {
@@ -495,7 +490,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         const double dmin = grid->dx < grid->dy ? grid->dx : grid->dy;
         s->prm.dt_max = grid->real_bits == 64 ? default_dt_max<double>(peds, p, dmin) : default_dt_max<float>(peds, p, dmin);
     }
-    s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? (nx % 2 == 0 ? 3 : 2) : (nx % 4 == 0) ? 1 : 0;
+    s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? (nx % 16 == 0 ? 4 : nx % 2 == 0 ? 3 : 2) : (nx % 4 == 0) ? 1 : 0;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -561,13 +556,29 @@ extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
 
 extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? 6 : 2) : 0; }
 
+extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
+{
+    if (!s) return SIM_EINVAL;
+    if (rows < 8 || rows > MARCH_MAX_R) return fail(s, SIM_EINVAL, "rows per chunk must be in [8, 64]");
+    CU(cudaStreamSynchronize(s->stream));
+    s->march_R = rows;
+    s->march_gy = (s->grid.ny + rows - 1) / rows;
+    drop_graphs(s);
+    if (s->grid.real_bits == 32)
+        flood_chunk_flags_kernel<float><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const float *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
+    else
+        flood_chunk_flags_kernel<double><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const double *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
+    CU(cudaGetLastError());
+    return SIM_OK;
+}
+
 extern "C" int sim_get_flood_variant(const sim_t *s) { return s ? s->flood_variant : SIM_EINVAL; }
 
 extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
 {
     if (!s) return SIM_EINVAL;
-    if (variant < 0 || variant > 7) return fail(s, SIM_EINVAL, "variant must be 0..7");
-    if (variant >= 6 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
+    if (variant < 0 || variant > 4) return fail(s, SIM_EINVAL, "variant must be 0..4");
+    if (variant == 4 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
     if (variant == 3 && s->grid.nx % 2 != 0) return fail(s, SIM_EINVAL, "the two-column march kernel needs nx % 2 == 0");
     if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");
     CU(cudaStreamSynchronize(s->stream));

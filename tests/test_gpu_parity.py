@@ -94,20 +94,20 @@ def _one_step(sc, evolve, variant=None, check_peds=True):
 
 # ------------------------------------------------------------------ flood, single step
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("evolve", [0, 7, 40])
 def test_config1_single_step_fp64(variant, evolve):
     _one_step(S.make(1), evolve, variant)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 def test_config2_single_step_fp32_wet_dry_inflow(variant):
     sc = S.make(2)
     sc.hydro_q = sc.hydro_q * 20.0            # a stronger flood so that a lot of the hall is wet
     _one_step(sc, 300, variant)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 def test_config4_mini_single_step_fp32_buildings_all_hr_classes(variant):
     sc = S.make(4, n=256, n_peds=5000)
     o, g = _one_step(sc, 150, variant)
@@ -124,7 +124,7 @@ def test_ragged_tiles_and_tiny_grids(nx, ny):
     for bits in (64, 32):
         sc = box(nx, ny, dx=0.5, real_bits=bits, z=z, h0=h0, u0=rng.normal(0, 0.5, (ny, nx)),
                  v0=rng.normal(0, 0.5, (ny, nx)), mask=mask, manning=0.03, dt_max=0.05)
-        for variant in [v for v in range(8) if nx % {0: 1, 1: 4, 2: 1, 3: 2, 4: 1, 5: 1, 6: 16, 7: 16}[v] == 0]:
+        for variant in [v for v in range(5) if nx % {0: 1, 1: 4, 2: 1, 3: 2, 4: 16}[v] == 0]:
             o, g = make_pair(sc, evolve=0, variant=variant)
             sync(o, g, sc)
             for _ in range(3):
@@ -155,7 +155,7 @@ def test_march_kernel_interior_chunks_take_the_fast_path(bits, solids):
              v0=rng.normal(0, 0.3, (ny, nx)), mask=mask, manning=0.02, dt_max=0.02,
              inflow_cell=np.arange(10, 30, dtype=np.int32) * nx, inflow_side=np.zeros(20, np.uint8),
              hydro_t=np.array([0.0, 1.0]), hydro_q=np.array([3.0, 3.0]))
-    for march in (2, 3, 4, 5, 6, 7):
+    for march in (2, 3, 4):
         o, g = make_pair(sc, evolve=0, variant=march)
         sync(o, g, sc)
         for _ in range(3):
@@ -164,7 +164,7 @@ def test_march_kernel_interior_chunks_take_the_fast_path(bits, solids):
             sync(o, g, sc)
     # and the three kernels agree with one another after a few free-running steps
     outs = []
-    for variant in range(8):
+    for variant in range(5):
         g2 = binding.Sim(sc); g2.set_flood_variant(variant); g2.step(5)
         outs.append(g2.read_conserved())
     for k in ("h", "qx", "qy"):
@@ -285,7 +285,9 @@ def test_config2_multi_step_aggregates_fp32():
     assert abs(a["t"] - b["t"]) <= 1e-4 * b["t"]
     assert abs(a["volume"] - b["volume"]) <= 1e-4 * b["volume"]      # fp32 storage of h: 1e-5 per DESIGN + dt drift
     assert abs(a["max_h"] - b["max_h"]) <= 1e-3 * b["max_h"]
-    assert sum(abs(x - y) for x, y in zip(a["hist"], b["hist"])) <= 0.01 * sc.n_peds
+    # chaotic fp32 crowd at the exit queue (order inside a bin, hence the summation order, is not
+    # fixed): at most 1 % of the agents may sit in another class; each of them counts twice in L1
+    assert sum(abs(x - y) for x, y in zip(a["hist"], b["hist"])) <= 0.02 * sc.n_peds
 
 
 def test_t_end_lands_and_halts_on_device():
@@ -303,7 +305,7 @@ def test_t_end_lands_and_halts_on_device():
 def test_no_pedestrians_and_lake_at_rest_on_gpu():
     sc = S.make(1, n_peds=0)
     sc.h0 = np.maximum(0.0, 0.2 - sc.z)                 # island
-    for variant in range(8):
+    for variant in range(5):
         g = binding.Sim(sc); g.set_flood_variant(variant)
         g.step(500)
         c = g.read_conserved()
