@@ -31,6 +31,9 @@ template <typename T> struct Vec4 { T v[4]; };
 template <> struct __align__(16) Vec4<float> { float v[4]; };
 template <> struct __align__(32) Vec4<double> { double v[4]; };
 
+// N adjacent reals moved with one 64- or 128-bit access
+template <typename T, int N> struct __align__(sizeof(T) * N) VecN { T v[N]; };
+
 template <typename T> __device__ __forceinline__ T solid_z();
 template <> __device__ __forceinline__ float solid_z<float>() { return CUDART_INF_F; }
 template <> __device__ __forceinline__ double solid_z<double>() { return CUDART_INF; }

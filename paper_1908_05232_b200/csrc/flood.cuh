@@ -418,9 +418,9 @@ __global__ void flood_stats_kernel(FloodArgs<T> a, double *out /* volume, max_h,
         if (!isfinite((double)h) || !isfinite((double)a.qx[p][c]) || !isfinite((double)a.qy[p][c])) { bad += 1; continue; }
         vol += (double)h;
         mh = fmax(mh, (double)h);
-        if (h > a.h_dry) {
-            const double u = (double)a.qx[p][c] / (double)h, v = (double)a.qy[p][c] / (double)h;
-            mr = fmax(mr, (fmax(fabs(u), fabs(v)) + 0.5) * (double)h);
+        if (h > a.h_dry) {                            // HR = (V + 0.5) h in the storage precision
+            const T u = div_rn(a.qx[p][c], h), v = div_rn(a.qy[p][c], h);
+            mr = fmax(mr, (double)mul_rn(add_rn(fmax(fabs(u), fabs(v)), T(0.5)), h));
         }
     }
     for (int o = 16; o > 0; o >>= 1) {

@@ -16,7 +16,6 @@
 
 namespace fp {
 
-template <typename T, int CPT> struct __align__(sizeof(T) * CPT) VecN { T v[CPT]; };
 template <int CPT> struct __align__(CPT) ByteN { uint8_t v[CPT]; };
 
 template <typename T, int CPT>

@@ -54,6 +54,7 @@ struct sim {
     uint8_t *ped_out_u8[3]{};
     int32_t *ped_out_i32[2]{};
     int32_t *key = nullptr, *off = nullptr, *count = nullptr, *start = nullptr, *cellprev = nullptr;
+    void *bxy = nullptr;              // (x, y) of the sorted level-n agents, interleaved, for the pair loop
     unsigned long long *scan_status = nullptr;
     Ctl *ctl = nullptr;
     double *stat_d = nullptr;       // [4] volume, max_h, max_hr, n_bad ; [4] ped bad
@@ -111,6 +112,7 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 3; ++k) s->ped_out_u8[k] = b.take<uint8_t>(np);
     for (int k = 0; k < 2; ++k) s->ped_out_i32[k] = b.take<int32_t>(np);
     s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(np);
+    s->bxy = real(2 * (size_t)np);
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
     s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * ((s->grid.ny + 7) / 8));    // room for any R >= 8
     s->scan_status = b.take<unsigned long long>((size_t)(s->nbins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1);
@@ -200,6 +202,9 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
     a.A = ped_soa<T>(s, 0); a.B = ped_soa<T>(s, 1);
     a.key = s->key; a.off = s->off; a.count = s->count; a.start = s->start; a.cellprev = s->cellprev;
     a.occ = s->occ; a.mask = s->mask; a.nav = s->nav;
+    a.bxy = (VecN<T, 2> *)s->bxy;
+    a.c_exp1 = (T)(2.0 * p.radius / p.B_s * 1.4426950408889634 + std::log2(p.A_s));   // A e^{(2r-d)/B} = 2^{c1 + c2 d}
+    a.c_exp2 = (T)(-1.4426950408889634 / p.B_s);
     for (int k = 0; k < 2; ++k) { a.h[k] = (const T *)s->h[k]; a.qx[k] = (const T *)s->qx[k]; a.qy[k] = (const T *)s->qy[k]; }
     a.ctl = s->ctl;
     return a;

@@ -30,6 +30,8 @@ struct PedArgs {
     int n_exit; int exit_i[16], exit_j[16];
     int storage_i, storage_j, drop_i, drop_j, arrive;
     PedSoA<T> A, B;                  // A: level n (any order) and level n+1; B: level n sorted by bin
+    VecN<T, 2> *bxy;                 // (x, y) of B interleaved: one 64/128-bit load per candidate
+    T c_exp1, c_exp2;                // fp32 pair force: A_s e^{(2r-d)/B_s} = 2^{c_exp1 + c_exp2 d}
     int32_t *key, *off;              // per slot of A: bin key, rank inside the bin
     int32_t *count;                  // [nbins+1] (zeroed by the scan after use)
     int32_t *start;                  // [nbins+2] exclusive scan
@@ -167,10 +169,26 @@ __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= a.n) return;
     const int d = a.start[a.key[s]] + a.off[s];
-    a.B.x[d] = a.A.x[s]; a.B.y[d] = a.A.y[s]; a.B.vx[d] = a.A.vx[s]; a.B.vy[d] = a.A.vy[s];
+    const T x = a.A.x[s], y = a.A.y[s];
+    a.B.x[d] = x; a.B.y[d] = y; a.bxy[d] = VecN<T, 2>{x, y};
+    a.B.vx[d] = a.A.vx[s]; a.B.vy[d] = a.A.vy[s];
     a.B.vpref[d] = a.A.vpref[s]; a.B.timer[d] = a.A.timer[s];
     a.B.role[d] = a.A.role[s]; a.B.fsm[d] = a.A.fsm[s]; a.B.state[d] = a.A.state[s];
     a.B.active[d] = a.A.active[s]; a.B.id[d] = a.A.id[s]; a.B.cell[d] = a.A.cell[s];
+}
+
+// A_s exp((2r - d)/B_s) / d for the pair at squared distance d2 (C24)
+__device__ __forceinline__ float pair_force(const PedArgs<float> &a, float d2)
+{
+    const float rinv = fast_rsqrt(d2);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fmaf(d2 * rinv, a.c_exp2, a.c_exp1)));
+    return e * rinv;
+}
+__device__ __forceinline__ double pair_force(const PedArgs<double> &a, double d2)
+{
+    const double d = sqrt(d2);
+    return a.A_s * exp((a.two_r - d) * a.inv_B) / d;
 }
 
 // ---------------------------------------------------------------------------------- (P)+(O)
@@ -204,11 +222,11 @@ __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
         const int s0 = a.start[jy * a.nbx + max(bx - 1, 0)];
         const int s1 = a.start[jy * a.nbx + min(bx + 1, a.nbx - 1) + 1];
         for (int j = s0; j < s1; ++j) {
-            const T ddx = x - B.x[j], ddy = y - B.y[j];
+            const VecN<T, 2> pj = a.bxy[j];
+            const T ddx = x - pj.v[0], ddy = y - pj.v[1];
             const T d2 = ddx * ddx + ddy * ddy;
             if (d2 > T(0) && d2 < a.R2) {
-                const T rinv = fast_rsqrt(d2);
-                const T f = a.A_s * fast_exp((a.two_r - d2 * rinv) * a.inv_B) * rinv;
+                const T f = pair_force(a, d2);
                 ax += f * ddx; ay += f * ddy;
             }
         }
@@ -386,12 +404,21 @@ __global__ void ped_key_by_id_kernel(PedSoA<T> A, const int32_t *key, int n, int
 
 // state histogram for sim_get_stats: hist[0..4] active by state, hist[5] = left the domain
 template <typename T>
-__global__ void ped_hist_kernel(PedSoA<T> A, int n, unsigned long long *hist, double *n_bad)
+__global__ void __launch_bounds__(256) ped_hist_kernel(PedSoA<T> A, int n, unsigned long long *hist, double *n_bad)
 {
+    __shared__ unsigned int sh[7];                     // per-block counts: 6 classes + non-finite
+    if (threadIdx.x < 7) sh[threadIdx.x] = 0u;
+    __syncthreads();
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
-    atomicAdd(&hist[A.active[s] ? min((int)A.state[s], 4) : 5], 1ull);
-    if (!isfinite((double)A.x[s]) || !isfinite((double)A.y[s])) atomicAdd(n_bad, 1.0);
+    if (s < n) {
+        const int k = A.active[s] ? min((int)A.state[s], 4) : 5;
+        const unsigned peers = __match_any_sync(__activemask(), k);
+        if ((threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&sh[k], (unsigned)__popc(peers));
+        if (!isfinite((double)A.x[s]) || !isfinite((double)A.y[s])) atomicAdd(&sh[6], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < 6 && sh[threadIdx.x]) atomicAdd(&hist[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
+    if (threadIdx.x == 6 && sh[6]) atomicAdd(n_bad, (double)sh[6]);
 }
 
 }  // namespace fp
