@@ -152,6 +152,8 @@ def run_ours(args):
     g = binding.Sim(sc, device=f"cuda:{local}")
     if args.flood_variant >= 0:
         g.set_flood_variant(args.flood_variant)
+    if args.no_overlap:
+        g.set_overlap(False)
     variant = g.flood_variant()
     kps = g.kernels_per_step()
 
@@ -190,7 +192,7 @@ def run_ours(args):
     KP = min(K, 100)
     kms = g.step_profiled(KP)
     flood_ms = kms["flood_step"] / KP
-    ped_ms = (kms["bin_count"] + kms["bin_scan"] + kms["scatter"] + kms["ped_step"]) / KP
+    ped_ms = (kms["bin_count"] + kms["bin_scan"] + kms["scatter"] + kms["occupancy"] + kms["ped_step"]) / KP
     peak, peak_src = peaks()
     fb = FLOOD_BYTES_PER_CELL if sc.real_bits == 32 else 65
     flood_gbs = ncell * fb / (flood_ms * 1e-3) / 1e9
@@ -254,7 +256,7 @@ def run_ours(args):
         "config": {"workload": f"config{args.config}: {sc.name}", "nx": sc.nx, "ny": sc.ny, "dx": sc.dx,
                    "pedestrians": npeds, "active_pedestrians": active,
                    "l2_policy": "inputs larger than L2 (no flush)" if ncell * fb > 126e6 else "working set fits L2: latency-bound config, roofline not meaningful",
-                   "flood_variant": variant, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+                   "flood_variant": variant, "overlap_ped_flood": not args.no_overlap, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": world * ncell * e2e_done / e2e_s, "unit": "cell-updates/s",
                 "h2d_bytes_per_step": h2d / e2e_done, "d2h_bytes_per_step": d2h / e2e_done,
@@ -267,7 +269,7 @@ def run_ours(args):
                      "bytes_per_cell": fb, "kernel_ms": flood_ms, "traffic": None,
                      "timed_with": f"cudaEvent before each launch over {KP} steps (sim_step_profiled) right after the timed region"},
         "kernels_ms_per_step": {k: v / KP for k, v in kms.items()},
-        "ped_roofline": {"bound": "hbm", "kernels": "bin_count+bin_scan+scatter+ped_step", "achieved": ped_gbs, "peak": peak,
+        "ped_roofline": {"bound": "hbm", "kernels": "bin_count+bin_scan+scatter+occupancy+ped_step", "achieved": ped_gbs, "peak": peak,
                          "unit": "GB/s", "frac": ped_gbs / peak, "ms": ped_ms},
         "cpu_baseline": cpu,
         "final": {"t": st1["t"], "volume": st1["volume"], "max_h": st1["max_h"], "hist": st1["hist"],
@@ -287,6 +289,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--flood-variant", type=int, default=-1, choices=list(range(-1, 5)), help="-1: the library default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-overlap", action="store_true", help="pedestrian step and flood step in one chain instead of parallel graph branches")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

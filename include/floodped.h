@@ -147,7 +147,7 @@ int sim_step(sim_t *s, int64_t n);
 
 /* The same n steps launched kernel by kernel (no graph) with a CUDA event before each launch;
  * synchronises.  kernel_ms[8] receives the summed device time in ms of: 0 bin count, 1 bin scan,
- * 2 scatter, 3 pedestrian step, 4 flood step, 5 tail; 6, 7 unused.  For measurement. */
+ * 2 scatter, 3 pedestrian step, 4 flood step, 5 tail, 6 occupancy (N_p per cell); 7 unused.  For measurement. */
 int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms);
 
 /* Flood agents' recorded fields: depth, velocities (0 where h <= h_dry, C8), bed,
@@ -186,6 +186,9 @@ int sim_set_flood_variant(sim_t *s, int32_t variant);
 int sim_get_flood_variant(const sim_t *s);         /* the kernel in use, or SIM_EINVAL */
 /* Rows per chunk of the row-marching kernels (8..64; default chosen by sim_create). Tuning hook. */
 int sim_set_march_rows(sim_t *s, int32_t rows);
+/* 1 (default): the pedestrian step runs as a parallel branch of the step graph beside the flood
+ * step (both read level n only); 0: every kernel of the step in one chain.  Same results. */
+int sim_set_overlap(sim_t *s, int32_t on);
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
 

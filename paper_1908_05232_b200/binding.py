@@ -19,7 +19,7 @@ SIM_OK, SIM_EINVAL, SIM_ENOMEM, SIM_ECUDA, SIM_ENOTFINITE = 0, -1, -2, -3, -4
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
-    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows",
+    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap",
     "sim_kernels_per_step", "sim_last_error", "sim_destroy",
 ]
 
@@ -111,6 +111,7 @@ def load_library(path: str = LIB_PATH):
     L.sim_set_flood_variant.argtypes = [_vp, C.c_int32]
     L.sim_get_flood_variant.argtypes = [_vp]
     L.sim_set_march_rows.argtypes = [_vp, C.c_int32]
+    L.sim_set_overlap.argtypes = [_vp, C.c_int32]
     L.sim_kernels_per_step.argtypes = [_vp]
     L.sim_last_error.argtypes = [_vp]
     L.sim_last_error.restype = C.c_char_p
@@ -240,7 +241,7 @@ class Sim:
     def step(self, n=1):
         self._chk(self._L.sim_step(self._h, int(n)))
 
-    KERNELS = ("bin_count", "bin_scan", "scatter", "ped_step", "flood_step", "tail")
+    KERNELS = ("bin_count", "bin_scan", "scatter", "ped_step", "flood_step", "tail", "occupancy")
 
     def step_profiled(self, n=1) -> dict:
         """n steps with per-kernel CUDA-event timing; returns summed ms per kernel."""
@@ -256,6 +257,9 @@ class Sim:
 
     def set_march_rows(self, rows):
         self._chk(self._L.sim_set_march_rows(self._h, int(rows)))
+
+    def set_overlap(self, on):
+        self._chk(self._L.sim_set_overlap(self._h, int(bool(on))))
 
     def flood_variant(self) -> int:
         return self._L.sim_get_flood_variant(self._h)

@@ -64,6 +64,9 @@ struct sim {
     uint8_t *chunk_flag = nullptr;
     int exit_i[16]{}, exit_j[16]{};
     cudaGraphExec_t graph1 = nullptr, graphN = nullptr;
+    cudaStream_t stream2 = nullptr;   // second branch of the step graph (pedestrian step beside the flood step)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int overlap = 1;
     std::string err;
 };
 
@@ -230,6 +233,8 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
     pa.n_exit = s->prm.n_exit_cells;
     int k = 0;
     auto mark = [&]() { if (ev) cudaEventRecord(ev[k++], st); };     // profiling mode only
+    // flood and pedestrian step both read level n only: in graph mode they run as parallel branches
+    const bool fork = !ev && s->np > 0 && s->overlap;
     if (s->np > 0) {
         const int nb = (s->np + 255) / 256;
         mark();
@@ -240,8 +245,17 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
         mark();
         ped_scatter_kernel<T><<<nb, 256, 0, st>>>(pa);
         mark();
-        ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, st>>>(pa);
-    } else k = 4;
+        ped_occ_kernel<T><<<nb, 256, 0, st>>>(pa);
+        mark();
+        if (fork) {
+            CU(cudaEventRecord(s->ev_fork, st));
+            CU(cudaStreamWaitEvent(s->stream2, s->ev_fork, 0));
+            ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, s->stream2>>>(pa);
+            CU(cudaEventRecord(s->ev_join, s->stream2));
+        } else {
+            ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, st>>>(pa);
+        }
+    } else k = 5;
     FloodArgs<T> fa = flood_args<T>(s);
     mark();
     if (s->flood_variant == 4) {
@@ -258,6 +272,7 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
         flood_cell_kernel<T><<<grid, blk, 0, st>>>(fa);
     }
     mark();
+    if (fork) CU(cudaStreamWaitEvent(st, s->ev_join, 0));
     tail_kernel<T><<<1, 32, 0, st>>>(tail_args<T>(s), 0);
     mark();
     CU(cudaGetLastError());
@@ -267,7 +282,8 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
 // n steps launched kernel by kernel with an event before each launch: per-kernel device time
 template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
 {
-    constexpr int NE = 7, BATCH = 64;
+    constexpr int NE = 8, BATCH = 64;
+    static const int slot_of[NE - 1] = {0, 1, 2, 6, 3, 4, 5};       // launch order -> kernel_ms index
     std::vector<cudaEvent_t> ev(NE * BATCH);
     for (auto &e : ev) CU(cudaEventCreate(&e));
     for (int k = 0; k < 8; ++k) ms[k] = 0.0;
@@ -278,12 +294,12 @@ template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
         if (rc != SIM_OK) break;
         cudaError_t e = cudaStreamSynchronize(s->stream);
         if (e != cudaSuccess) { rc = fail(s, SIM_ECUDA, cudaGetErrorString(e)); break; }
-        const int first = s->np > 0 ? 0 : 4;
+        const int first = s->np > 0 ? 0 : 5;
         for (int i = 0; i < m; ++i)
             for (int k = first; k < NE - 1; ++k) {
                 float t = 0.f;
                 cudaEventElapsedTime(&t, ev[(size_t)i * NE + k], ev[(size_t)i * NE + k + 1]);
-                ms[k] += t;
+                ms[slot_of[k]] += t;
             }
         n -= m;
     }
@@ -513,6 +529,9 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     auto run = [&]() -> int {
         CU(cudaMemsetAsync(s->ws, 0, s->ws_bytes, s->stream));
         CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&s->stream2, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
         int r = DISPATCH(s, upload_state, s, topo, manning, peds, p);
         if (r != SIM_OK) return r;
         for (int k = 0; k < 4; ++k) if (upload(s, s->inflow[k], infl[k].data(), infl[k].size())) return SIM_ECUDA;
@@ -559,7 +578,7 @@ extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
     return DISPATCH(s, step_profiled, s, n, kernel_ms);
 }
 
-extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? 6 : 2) : 0; }
+extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? 7 : 2) : 0; }
 
 extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
 {
@@ -574,6 +593,15 @@ extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
     else
         flood_chunk_flags_kernel<double><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const double *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
     CU(cudaGetLastError());
+    return SIM_OK;
+}
+
+extern "C" int sim_set_overlap(sim_t *s, int32_t on)
+{
+    if (!s) return SIM_EINVAL;
+    CU(cudaStreamSynchronize(s->stream));
+    s->overlap = on ? 1 : 0;
+    drop_graphs(s);
     return SIM_OK;
 }
 
@@ -868,6 +896,9 @@ extern "C" void sim_destroy(sim_t *s)
     if (s->ws) cudaStreamSynchronize(s->stream);
     drop_graphs(s);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
+    if (s->stream2) cudaStreamDestroy(s->stream2);
+    if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+    if (s->ev_join) cudaEventDestroy(s->ev_join);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
 }

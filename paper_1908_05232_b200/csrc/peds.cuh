@@ -177,6 +177,27 @@ __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
     a.B.active[d] = a.A.active[s]; a.B.id[d] = a.A.id[s]; a.B.cell[d] = a.A.cell[s];
 }
 
+// ---------------------------------------------------------------------------------- (O)
+// N_p per cell from the sorted level-n agents: the agents of a cell all sit in one bin, so
+// each agent counts those of its own bin that share its cell and the lowest slot publishes the
+// count.  Also remembers the cell so that next step's bin count can clear it (sparse clear).
+// Runs before the flood kernel, which consumes occ[]; the pedestrian step itself does not need it.
+template <typename T>
+__global__ void __launch_bounds__(256) ped_occ_kernel(PedArgs<T> a)
+{
+    if (a.ctl->halt) return;
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d >= a.n) return;
+    if (!a.B.active[d]) { a.cellprev[d] = -1; return; }
+    const int c = a.B.cell[d];
+    const int b = ((c / a.nx) / a.kbin) * a.nbx + (c % a.nx) / a.kbin;
+    int same = 0, lower = 0;
+    for (int j = a.start[b]; j < a.start[b + 1]; ++j)
+        if (a.B.cell[j] == c) { same += 1; lower += (j < d); }
+    if (lower == 0) a.occ[c] = (uint8_t)min(same, 255);
+    a.cellprev[d] = c;
+}
+
 // A_s exp((2r - d)/B_s) / d for the pair at squared distance d2 (C24)
 __device__ __forceinline__ float pair_force(const PedArgs<float> &a, float d2)
 {
@@ -193,6 +214,7 @@ __device__ __forceinline__ double pair_force(const PedArgs<double> &a, double d2
 
 // ---------------------------------------------------------------------------------- (P)+(O)
 // One thread per sorted slot d: reads level n from B (+ flood level n), writes level n+1 to A[d].
+// Independent of the flood kernel of the same step (both read level n), so the two may overlap.
 template <typename T>
 __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
 {
@@ -209,7 +231,6 @@ __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
     if (!act) {
         A.x[d] = x; A.y[d] = y; A.vx[d] = vx; A.vy[d] = vy; A.timer[d] = timer;
         A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 0;
-        a.cellprev[d] = -1;
         return;
     }
     const int ix = c % a.nx, iy = c / a.nx;
@@ -231,17 +252,6 @@ __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
             }
         }
     }
-    // N_p of my cell: agents of my own bin that share my cell
-    int same = 0, lower = 0;
-    {
-        const int b = by * a.nbx + bx;
-        for (int j = a.start[b]; j < a.start[b + 1]; ++j)
-            if (B.cell[j] == c) { same += 1; lower += (j < d); }
-    }
-    // (O) one agent per occupied cell publishes N_p; remember the cell for next step's clear
-    if (lower == 0) a.occ[c] = (uint8_t)min(same, 255);
-    a.cellprev[d] = c;
-
     // 8. exit (C29): level-n cell within arrive_cells of an exit cell
     if (role == 0 || fsm == 0) {
         bool out = false;
