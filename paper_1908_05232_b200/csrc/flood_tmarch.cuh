@@ -44,6 +44,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
                      : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     } while (!ok);
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t ok;
+    asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok));
+    return ok != 0;
+}
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -67,14 +77,23 @@ __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, 
 }
 
 // interior chunk (no domain edge, no solid cell in it or in its halo): rows y0-1 .. y0+R all exist
+//
+//   Synchronisation per row: the neighbour exchange (last-column state st[b], west-face flux
+//   fx[b]) goes through a SPLIT-PHASE barrier -- every thread arrives on xbar[b] right after
+//   publishing its state and waits only after the south faces, which need nothing from the
+//   neighbours, so the warp that also feeds the TMA ring no longer holds the others at a
+//   __syncthreads.  The ring slot is refilled after that wait (all threads have their values in
+//   registers before they arrive).  The TMA issue sits in a warp-uniform branch with one elected
+//   lane, its addresses derived from uniform values only.
 template <typename T, int CPT, int STAGES>
 __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, CPT> &s, RowStage<T> *ring,
                                           uint64_t *bars, int x0, int y0, int R)
 {
     constexpr int NT = MW / CPT;
     const int tid = threadIdx.x;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);       // warp-uniform by construction
     const int nx = a.nx;
-    const int p = a.ctl->parity;
+    const int p = __shfl_sync(0xffffffffu, a.ctl->parity, 0);
     const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
     const T *__restrict__ Z = a.zs;
     T *__restrict__ Ho = a.h[p ^ 1], *__restrict__ QXo = a.qx[p ^ 1], *__restrict__ QYo = a.qy[p ^ 1];
@@ -84,14 +103,18 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     const int i = x0 + tid * CPT;
     const int y1 = y0 + R;
     const int nrows = R + 2;                           // ring row r holds grid row y0 - 1 + r
+    uint64_t *xbar = bars + STAGES;                    // exchange barriers, by row parity
 
     if (tid == 0) {
         for (int k = 0; k < STAGES; ++k) mbar_init(&bars[k], 1);
+        mbar_init(&xbar[0], NT); mbar_init(&xbar[1], NT);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (tid == 0)
-        for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row(a, H, QX, QY, ring[r], &bars[r], x0, y0 - 1 + r);
+    if (warp == 0) {
+        if (elect_one())
+            for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row(a, H, QX, QY, ring[r], &bars[r], x0, y0 - 1 + r);
+    }
 
     // ---- pre-pass: strip-edge data for every row of the chunk (as in variants 2, 3)
     for (int k = tid; k < R; k += NT) {
@@ -125,7 +148,9 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         }
     }
     __syncthreads();                                   // slot 0 consumed; er/sw visible
-    if (tid == 0 && STAGES < nrows) tm_issue_row(a, H, QX, QY, ring[0], &bars[0], x0, y0 - 1 + STAGES);
+    if (warp == 0 && STAGES < nrows) {
+        if (elect_one()) tm_issue_row(a, H, QX, QY, ring[0], &bars[0], x0, y0 - 1 + STAGES);
+    }
 
     T ah[CPT], ax[CPT], ay[CPT], n0_p[CPT];
     int occ_p[CPT];
@@ -135,6 +160,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     int clamp_n = 0;
     int slot = 1 % STAGES;
     uint32_t phase = (1 / STAGES) & 1;
+    bool live_p = true;                                // anything but exact zeros in the accumulators?
 
 #pragma unroll 2
     for (int jj = y0; jj <= y1; ++jj) {
@@ -157,9 +183,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         const int b = jj & 1;
         s.st[b][0][tid] = eta[CPT - 1]; s.st[b][1][tid] = u[CPT - 1];
         s.st[b][2][tid] = v[CPT - 1];   s.st[b][3][tid] = z[CPT - 1];
-        __syncthreads();
-        if (tid == 0 && r + STAGES < nrows) tm_issue_row(a, H, QX, QY, ring[slot], &bars[slot], x0, y0 - 1 + r + STAGES);
-        if (++slot == STAGES) { slot = 0; phase ^= 1u; }
+        mbar_arrive(&xbar[b]);                         // publishes st[b] of this row and fx[b^1] of the previous one
 
         // south faces of the current row = north faces of the previous one (normal velocity v)
         T g0[CPT], g1L[CPT], g1R[CPT], g2[CPT];
@@ -167,17 +191,32 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         for (int k = 0; k < CPT; ++k)
             face_eta<T, false, true>(g, eta_p[k], v_p[k], u_p[k], z_p[k], eta[k], v[k], u[k], z[k], g0[k], g1L[k], g1R[k], g2[k]);
 
+        mbar_wait(&xbar[b], (uint32_t)((jj - y0) >> 1) & 1u);
+        if (warp == 0 && r + STAGES < nrows) {
+            if (elect_one()) tm_issue_row(a, H, QX, QY, ring[slot], &bars[slot], x0, y0 - 1 + r + STAGES);
+        }
+        if (++slot == STAGES) { slot = 0; phase ^= 1u; }
+
         if (jj > y0) {                                 // finish row jj-1
             const int j = jj - 1, bp = b ^ 1;
             const T *fe = (tid == NT - 1) ? &s.er[0][j - y0] : &s.fx[bp][0][tid + 1];
             const int stride = (tid == NT - 1) ? MARCH_MAX_R : NT;
+            const T e0 = fe[0], e1 = fe[stride], e2 = fe[2 * stride];
+            // a warp whose cells of this row hold exact zeros and receive no flux writes zeros
+            bool live = live_p || e0 != T(0) || e1 != T(0) || e2 != T(0);
+#pragma unroll
+            for (int k = 0; k < CPT; ++k) live = live || g0[k] != T(0) || g1L[k] != T(0) || g2[k] != T(0);
             VecN<T, CPT> ho, qxo, qyo;
 #pragma unroll
-            for (int k = 0; k < CPT; ++k) {
-                T hn = ah[k] - dtdy * g0[k], qxn = ax[k] - dtdy * g2[k], qyn = ay[k] - dtdy * g1L[k];
-                if (k == CPT - 1) { hn -= dtdx * fe[0]; qxn -= dtdx * fe[stride]; qyn -= dtdx * fe[2 * stride]; }
-                finish_hat2(a, dt, hn, qxn, qyn, n0_p[k], occ_p[k], lam, clamp_h, clamp_n);
-                ho.v[k] = hn; qxo.v[k] = qxn; qyo.v[k] = qyn;
+            for (int k = 0; k < CPT; ++k) { ho.v[k] = qxo.v[k] = qyo.v[k] = T(0); }
+            if (__any_sync(0xffffffffu, live)) {
+#pragma unroll
+                for (int k = 0; k < CPT; ++k) {
+                    T hn = ah[k] - dtdy * g0[k], qxn = ax[k] - dtdy * g2[k], qyn = ay[k] - dtdy * g1L[k];
+                    if (k == CPT - 1) { hn -= dtdx * e0; qxn -= dtdx * e1; qyn -= dtdx * e2; }
+                    finish_hat2(a, dt, hn, qxn, qyn, n0_p[k], occ_p[k], lam, clamp_h, clamp_n);
+                    ho.v[k] = hn; qxo.v[k] = qxn; qyo.v[k] = qyn;
+                }
             }
             const size_t c = (size_t)j * nx + i;
             *reinterpret_cast<VecN<T, CPT> *>(Ho + c) = ho;
@@ -195,12 +234,14 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 face_eta<T, false, true>(g, eta[k - 1], u[k - 1], v[k - 1], z[k - 1], eta[k], u[k], v[k], z[k],
                                          f0[k], f1L[k], f1R[k], f2[k]);
             s.fx[b][0][tid] = f0[0]; s.fx[b][1][tid] = f1L[0]; s.fx[b][2][tid] = f2[0];
+            live_p = false;
 #pragma unroll
             for (int k = 0; k < CPT; ++k) {
                 ah[k] = hc[k] + dtdx * f0[k] + dtdy * g0[k];
                 ax[k] = qxc[k] + dtdx * f1R[k] + dtdy * g2[k];
                 ay[k] = qyc[k] + dtdx * f2[k] + dtdy * g1R[k];
                 if (k < CPT - 1) { ah[k] -= dtdx * f0[k + 1]; ax[k] -= dtdx * f1L[k + 1]; ay[k] -= dtdx * f2[k + 1]; }
+                live_p = live_p || ah[k] != T(0) || ax[k] != T(0) || ay[k] != T(0);
             }
         }
 #pragma unroll
@@ -216,7 +257,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     return lam;
 }
 
-template <typename T, int STAGES> constexpr size_t tmarch_dyn_smem() { return sizeof(RowStage<T>) * STAGES + 8 * STAGES + 16; }
+template <typename T, int STAGES> constexpr size_t tmarch_dyn_smem() { return sizeof(RowStage<T>) * STAGES + 8 * (STAGES + 2) + 16; }
 
 template <typename T, int CPT, int STAGES, int MINB>
 __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tmarch_kernel(FloodArgs<T> a)

@@ -451,6 +451,74 @@ def throughput_stress(n: int = 8192, n_peds: int = 1_000_000, steps: int = 500, 
         steps=steps)
 
 
+# --------------------------------------------------------------------------- mid-run states
+
+def synthetic_flow(sc: Scenario, seed: int, speed: float = 1.5, ped_speed: float = 1.0) -> dict:
+    """A seeded state that looks like the middle of a run, for single-step parity at sizes the
+    oracle cannot evolve itself: the scenario's initial depth modulated by +-20 % smooth noise,
+    smooth velocities in [-speed, speed] m/s (conserved variables q = h * u rounded to storage
+    precision), pedestrians with uniform random velocities of up to ped_speed.  Input generation
+    only; nothing here is the method's arithmetic."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    ny, nx = sc.ny, sc.nx
+    sp = [max(2, nx // 32), max(2, nx // 128)]
+
+    def smooth():
+        return (_value_noise(rng, ny, nx, sp, [1.0, 0.5]).astype(np.float32) - np.float32(0.5)) * np.float32(2.0)
+
+    h = sc.h0.reshape(ny, nx).astype(np.float32) * (np.float32(1.0) + np.float32(0.2) * smooth())
+    h = np.where(sc.mask.reshape(ny, nx) != 0, np.float32(0.0), h).astype(np.float32)
+    qx = (h * (np.float32(speed) * smooth())).astype(np.float32)
+    qy = (h * (np.float32(speed) * smooth())).astype(np.float32)
+    n = sc.n_peds
+    ang = rng.random(n) * 2.0 * np.pi
+    mag = rng.random(n) * ped_speed
+    real = sc.real
+    return dict(h=h.reshape(-1).astype(real), qx=qx.reshape(-1).astype(real), qy=qy.reshape(-1).astype(real),
+                pvx=(mag * np.cos(ang)).astype(real), pvy=(mag * np.sin(ang)).astype(real))
+
+
+def window(sc: Scenario, state: dict, i0: int, j0: int, w: int, hgt: int):
+    """The sub-box [i0, i0+w) x [j0, j0+hgt) of a scenario and of a state of it as a Scenario of
+    its own (closed walls; inflow faces kept where the window touches the inflow edge, the
+    hydrograph scaled so that the discharge per unit width is unchanged; pedestrians inside the
+    window, coordinates shifted by a whole number of cells).  Returns (scenario, state, ids):
+    ids = indices of the window's pedestrians in the parent.  One first-order step of the parent
+    restricted to the window's interior depends on nothing outside the window."""
+    nx, ny = sc.nx, sc.ny
+    sl = np.s_[j0:j0 + hgt, i0:i0 + w]
+
+    def cut(a, dtype=None):
+        a = np.asarray(a).reshape(ny, nx)[sl].reshape(-1)
+        return np.ascontiguousarray(a if dtype is None else a.astype(dtype))
+
+    ci, cj = (sc.px / sc.dx).astype(np.int64), (sc.py / sc.dy).astype(np.int64)
+    ids = np.flatnonzero((ci >= i0) & (ci < i0 + w) & (cj >= j0) & (cj < j0 + hgt))
+    real = sc.real
+    ox, oy = real(i0) * real(sc.dx), real(j0) * real(sc.dy)
+    keep = [k for k, c in enumerate(sc.exit_cells)
+            if i0 <= c % nx < i0 + w and j0 <= c // nx < j0 + hgt]
+    exits = np.array([(sc.exit_cells[k] // nx - j0) * w + (sc.exit_cells[k] % nx - i0) for k in keep], np.int32)
+    fi, fj = sc.inflow_cell % nx, sc.inflow_cell // nx
+    fk = np.flatnonzero((fi >= i0) & (fi < i0 + w) & (fj >= j0) & (fj < j0 + hgt))
+    nav = np.stack([cut(sc.nav_dir[t]) for t in range(sc.nav_dir.shape[0])])
+    scale = fk.size / max(sc.inflow_cell.size, 1)
+    sub = Scenario(
+        name=f"{sc.name}[{i0}:{i0 + w},{j0}:{j0 + hgt}]", nx=w, ny=hgt, dx=sc.dx, dy=sc.dy, real_bits=sc.real_bits,
+        z=cut(sc.z), manning=cut(sc.manning), mask=cut(sc.mask), h0=cut(state["h"]), u0=None, v0=None,
+        px=(sc.px[ids] - ox).astype(real), py=(sc.py[ids] - oy).astype(real),
+        pvx=np.ascontiguousarray(state["pvx"][ids]), pvy=np.ascontiguousarray(state["pvy"][ids]),
+        pvpref=np.ascontiguousarray(sc.pvpref[ids]), prole=np.ascontiguousarray(sc.prole[ids]),
+        nav_dir=nav, exit_cells=exits,
+        g=sc.g, cfl=sc.cfl, dt_max=sc.dt_max, h_dry=sc.h_dry, couple_roughness=sc.couple_roughness, n_cap=sc.n_cap,
+        inflow_cell=((fj[fk] - j0) * w + (fi[fk] - i0)).astype(np.int32), inflow_side=np.ascontiguousarray(sc.inflow_side[fk]),
+        hydro_t=sc.hydro_t.copy(), hydro_q=sc.hydro_q * scale,
+        hr_edges=sc.hr_edges, speed_wet=sc.speed_wet, tau=sc.tau, A_s=sc.A_s, B_s=sc.B_s, radius=sc.radius,
+        R_int=sc.R_int, vmax_factor=sc.vmax_factor, arrive_cells=sc.arrive_cells)
+    sub_state = dict(h=cut(state["h"]), qx=cut(state["qx"]), qy=cut(state["qy"]))
+    return sub, sub_state, ids
+
+
 CONFIGS = {
     1: tiny_dam_break,
     2: shopping_centre,

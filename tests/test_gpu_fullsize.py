@@ -1,0 +1,178 @@
+"""GPU parity at BASELINE.json's FULL sizes (Config 4: 2048^2 cells + 1e5 pedestrians, Config 5:
+8192^2 cells + 1e6 pedestrians), in the launch configuration bench.py times (library defaults:
+TMA row-marching flood kernel, CUDA graph, pedestrian step beside the flood step).
+
+The oracle cannot run these sizes in a test, but one first-order coupled step of a cell depends
+only on its four neighbours and one step of a pedestrian only on agents within R_int, so the
+oracle recomputes SAMPLED WINDOWS one by one: each window of the seeded full-size state becomes a
+small closed box (scenarios.window) that the oracle steps once; the window's interior cells and
+core pedestrians must match the full-size CUDA result element by element (floats 1e-5 in the
+mixed norm, integers exact).  Every oracle input comes from the seeded generators
+(scenarios.make + scenarios.synthetic_flow), none from the CUDA path.  What windows cannot see
+(the global CFL reduction, total volume) is checked as a property of the full output."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1908_05232_b200 import binding, scenarios as S
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+W = 64                     # window edge in cells
+T0 = 30.0                  # Config 5's inflow ramp is at half height
+
+
+def _windows(sc, rng, n_random):
+    nx, ny = sc.nx, sc.ny
+    wins = [(0, 0), (nx - W, 0), (0, ny - W), (nx - W, ny - W),          # domain corners
+            (nx // 2 - W // 2, 0), (nx // 2 - W // 2, ny - W),            # south (inflow, exit) / north edge
+            (0, ny // 2 - W // 2), (nx - W, ny // 2 - W // 2),            # west / east exit
+            (256 - W // 2, 64 - W // 2), (512 - W // 2, 37),              # straddling strip / chunk borders
+            (nx - 256 - W // 2, ny - 64 - W // 2)]
+    # densest crowd spots: windows centred on the busiest coarse cells
+    ci = np.clip((sc.px / sc.dx).astype(np.int64) // W, 0, nx // W - 1)
+    cj = np.clip((sc.py / sc.dy).astype(np.int64) // W, 0, ny // W - 1)
+    cnt = np.bincount(cj * (nx // W) + ci, minlength=(nx // W) * (ny // W))
+    for b in np.argsort(cnt)[::-1][:3]:
+        wins.append((int(b % (nx // W)) * W, int(b // (nx // W)) * W))
+    # random windows; half of them on the wet/dry front (a window holding both dry and wet cells)
+    h = sc.h0.reshape(ny, nx)
+    tries = 0
+    while n_random > 0 and tries < 1000:
+        tries += 1
+        i0, j0 = int(rng.integers(0, nx - W)), int(rng.integers(0, ny - W))
+        frac = float((h[j0:j0 + W, i0:i0 + W] > 0).mean())
+        if n_random % 2 == 0 or 0.1 < frac < 0.9:
+            wins.append((i0, j0)); n_random -= 1
+    return wins
+
+
+def _force_magnitude_sum(sub, sc):
+    """S_i = sum over partners within R_int of |f_ij| = A_s exp((2r - d)/B_s) (C24): the
+    scale that fp32 rounding of the social-force sum is relative to."""
+    S_i = np.zeros(sub.n_peds)
+    if sub.n_peds > 1:
+        from scipy.spatial import cKDTree
+        x, y = sub.px.astype(np.float64), sub.py.astype(np.float64)
+        pr = cKDTree(np.c_[x, y]).query_pairs(sc.R_int, output_type="ndarray")
+        d = np.hypot(x[pr[:, 0]] - x[pr[:, 1]], y[pr[:, 0]] - y[pr[:, 1]])
+        f = sc.A_s * np.exp((2.0 * sc.radius - d) / sc.B_s)
+        np.add.at(S_i, pr[:, 0], f); np.add.at(S_i, pr[:, 1], f)
+    return S_i
+
+
+def _near_threshold(sub, R_int):
+    """pedestrians with a partner within rounding of the cut-off R_int (either side may count it)"""
+    skip = np.zeros(sub.n_peds, bool)
+    if sub.n_peds > 1:
+        from scipy.spatial import cKDTree
+        x, y = sub.px.astype(np.float64), sub.py.astype(np.float64)
+        t = cKDTree(np.c_[x, y])
+        for i, j in t.query_pairs(R_int * (1 + 1e-4)):
+            if abs(math.hypot(x[i] - x[j], y[i] - y[j]) - R_int) < 1e-4 * R_int:
+                skip[i] = skip[j] = True
+    return skip
+
+
+@pytest.mark.parametrize("cfg,n_random", [(4, 24), (5, 24)])
+def test_full_size_single_step_on_sampled_windows(cfg, n_random):
+    sc = S.make(cfg)
+    nx, ny = sc.nx, sc.ny
+    st = S.synthetic_flow(sc, seed=900 + cfg)
+    sc.pvx, sc.pvy = st["pvx"], st["pvy"]
+    g = binding.Sim(sc)                                   # library defaults = what bench.py times
+    assert g.flood_variant() == 4
+    hmax = float(st["h"].max())
+    umax = float(np.max(np.abs(st["qx"]) / np.maximum(st["h"], 1e-3))) + float(np.max(np.abs(st["qy"]) / np.maximum(st["h"], 1e-3)))
+    dt = float(np.float32(0.4 * sc.dx / (umax + math.sqrt(sc.g * hmax))))
+    g.write_flood(st["h"], st["qx"], st["qy"])
+    g.set_time(T0, dt)
+    g.step(1)
+    a = {k: v.reshape(ny, nx) for k, v in g.read_conserved().items()}
+    pa = g.read_peds()
+    occ = g.read_occupancy().reshape(ny, nx)
+    sa = g.stats()
+    assert sa["step"] == 1 and abs(sa["t"] - (T0 + dt)) <= 1e-9
+    scale = {k: max(float(np.max(np.abs(st[k]))), 1e-30) for k in ("h", "qx", "qy")}
+    vscale = max(float(np.max(np.hypot(pa["vx"], pa["vy"]))), 1e-30)
+    L = nx * sc.dx
+
+    rng = np.random.default_rng(cfg)
+    n_cells = n_agents = n_skipped = 0
+    worst = dict(h=0.0, qx=0.0, qy=0.0, v=0.0, x=0.0)
+    for (i0, j0) in _windows(sc, rng, n_random):
+        sub, ss, ids = S.window(sc, st, i0, j0, W, W)
+        o = oracle.Oracle(sub)
+        o.write_flood(*(ss[k].astype(np.float64) for k in ("h", "qx", "qy")))
+        o.set_time(T0, dt)
+        o.step(1)
+        b = {k: v.reshape(W, W) for k, v in o.read_conserved().items()}
+        # interior: a window side that is not a domain edge has a fictitious wall -> drop its ring
+        lo_i, hi_i = (0 if i0 == 0 else 1), (W if i0 + W == nx else W - 1)
+        lo_j, hi_j = (0 if j0 == 0 else 1), (W if j0 + W == ny else W - 1)
+        for k in ("h", "qx", "qy"):
+            d = np.abs(a[k][j0 + lo_j:j0 + hi_j, i0 + lo_i:i0 + hi_i].astype(np.float64) - b[k][lo_j:hi_j, lo_i:hi_i])
+            err = float(d.max()) / scale[k]
+            worst[k] = max(worst[k], err)
+            assert err <= TOL, (cfg, i0, j0, k, err)
+        n_cells += (hi_i - lo_i) * (hi_j - lo_j)
+        assert np.array_equal(occ[j0:j0 + W, i0:i0 + W].astype(np.int64),
+                              np.minimum(o.read_occupancy(), 255).reshape(W, W)), (i0, j0)
+        if ids.size:
+            pb = o.read_peds()
+            # core agents: every partner within R_int and every cell they can reach lies in the window
+            m = (math.ceil(sc.R_int / sc.dx) + 2) * sc.dx
+            x, y = sub.px.astype(np.float64), sub.py.astype(np.float64)
+            core = np.ones(ids.size, bool)
+            if i0 > 0: core &= x >= m
+            if i0 + W < nx: core &= x <= W * sc.dx - m
+            if j0 > 0: core &= y >= m
+            if j0 + W < ny: core &= y <= W * sc.dy - m
+            skip = _near_threshold(sub, sc.R_int)
+            # ... or landing within fp32 rounding (of the full-size coordinate) of a cell edge: the move
+            # rejection at a solid cell (C27) may then be decided differently and zero a velocity component
+            eps = 4.0 * float(np.spacing(np.float32(L)))
+            for xs, d in ((pa["x"][ids].astype(np.float64), sc.dx), (pb["x"] + i0 * sc.dx, sc.dx),
+                          (pa["y"][ids].astype(np.float64), sc.dy), (pb["y"] + j0 * sc.dy, sc.dy)):
+                skip |= np.abs(xs - np.round(xs / d) * d) < eps
+            c = np.flatnonzero(core)
+            assert np.array_equal(pa["active"][ids][c], pb["active"][c])
+            assert np.array_equal(pa["state"][ids][c], pb["state"][c])
+            assert np.array_equal(pa["fsm"][ids][c], pb["fsm"][c])
+            ev = np.maximum(np.abs(pa["vx"][ids] - pb["vx"]), np.abs(pa["vy"][ids] - pb["vy"])) / vscale
+            ex = np.maximum(np.abs(pa["x"][ids] - (pb["x"] + i0 * sc.dx)), np.abs(pa["y"][ids] - (pb["y"] + j0 * sc.dy))) / L
+            # fp32 sum of pair forces: each term carries <= 16 ulp (ex2/rsqrt.approx and the rounding of
+            # the exponent argument d/B_s <= 12.5), the sum is multiplied by dt
+            tol_v = TOL + 16.0 * 2.0 ** -23 * dt * _force_magnitude_sum(sub, sc) / vscale
+            bad = core & ((ev > tol_v) | (ex > TOL))
+            assert not np.any(bad & ~skip), (cfg, i0, j0, np.flatnonzero(bad & ~skip)[:8], float(ev[core].max()))
+            assert int((bad & skip).sum()) <= max(2, c.size // 200)
+            ok = core & ~skip
+            if ok.any():
+                worst["v"] = max(worst["v"], float((ev[ok] / tol_v[ok]).max()) * TOL); worst["x"] = max(worst["x"], float(ex[ok].max()))
+            n_agents += int(ok.sum()); n_skipped += int((core & skip).sum())
+        o.close()
+    assert n_cells >= 30 * (W - 2) ** 2 and n_agents >= 1000, (n_cells, n_agents)
+
+    # ---- properties of the whole output that no window sees
+    # (T) next dt = min(dt_max, CFL / max over wet cells of the NEW state (|u|+c)/dx, (|v|+c)/dy)
+    h64 = a["h"].astype(np.float64)
+    wet = h64 > sc.h_dry
+    hs = np.where(wet, h64, 1.0)
+    c = np.sqrt(sc.g * hs)
+    lam = np.where(wet, np.maximum((np.abs(a["qx"] / hs) + c) / sc.dx, (np.abs(a["qy"] / hs) + c) / sc.dy), 0.0).max()
+    assert abs(sa["dt"] - sc.cfl / lam) <= 10 * TOL * sa["dt"], (sa["dt"], sc.cfl / lam)
+    # mass: closed walls, so the volume changes by the inflow of this step (+ the accounted clamp) only
+    q_in = float(np.interp(T0, sc.hydro_t, sc.hydro_q)) if sc.hydro_t.size else 0.0
+    v0 = float(st["h"].astype(np.float64).sum()) * sc.dx * sc.dy
+    v1 = float(h64.sum()) * sc.dx * sc.dy
+    assert abs((v1 - v0) - (q_in * dt + sa["clamped_volume"])) <= 2e-7 * v0, (v1 - v0, q_in * dt, sa["clamped_volume"])
+    assert float(h64.min()) >= 0.0
+    # nothing moves in solid cells
+    solid = sc.mask.reshape(ny, nx) != 0
+    assert not np.any(a["h"][solid]) and not np.any(a["qx"][solid]) and not np.any(a["qy"][solid])
+    print(f"config{cfg}: {n_cells} cells, {n_agents} agents (+{n_skipped} near a threshold) compared; worst {worst}")
+    g.close()
