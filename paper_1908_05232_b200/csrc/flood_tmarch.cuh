@@ -16,7 +16,10 @@
 //   with plain loads.  Needs nx % 16 == 0 (16-byte alignment of every row segment).
 #pragma once
 
+#include <type_traits>
+
 #include "flood_march2.cuh"
+#include "flood_pk.cuh"
 
 namespace fp {
 
@@ -38,10 +41,13 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
+    // try_wait suspends the thread in hardware until the phase completes or the time hint (ns)
+    // runs out; without the hint it returns after a short system-dependent time and the loop
+    // spins through issue slots (ncu: 16 rounds per row on the exchange barrier)
     uint32_t ok;
     do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
-                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity), "r"(100000u) : "memory");
     } while (!ok);
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -158,31 +164,125 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     for (int k = 0; k < CPT; ++k) { ah[k] = ax[k] = ay[k] = n0_p[k] = T(0); occ_p[k] = 0; }
     T lam = T(0), clamp_h = T(0);
     int clamp_n = 0;
-    int slot = 1 % STAGES;
-    uint32_t phase = (1 / STAGES) & 1;
     bool live_p = true;                                // anything but exact zeros in the accumulators?
 
-#pragma unroll 2
-    for (int jj = y0; jj <= y1; ++jj) {
-        const int r = jj - y0 + 1;
-        mbar_wait(&bars[slot], phase);
-        const RowStage<T> &st = ring[slot];
-        const VecN<T, CPT> hv = *reinterpret_cast<const VecN<T, CPT> *>(&st.h[tid * CPT]);
-        const VecN<T, CPT> qxv = *reinterpret_cast<const VecN<T, CPT> *>(&st.qx[tid * CPT]);
-        const VecN<T, CPT> qyv = *reinterpret_cast<const VecN<T, CPT> *>(&st.qy[tid * CPT]);
-        const VecN<T, CPT> zv = *reinterpret_cast<const VecN<T, CPT> *>(&st.z[tid * CPT]);
-        const VecN<T, CPT> n0_c = *reinterpret_cast<const VecN<T, CPT> *>(&st.n0[tid * CPT]);
-        const ByteN<CPT> occ_c = *reinterpret_cast<const ByteN<CPT> *>(&st.occ[tid * CPT]);
+    // my addresses: the ring slot is followed by a running pointer (wraps after STAGES rows), the
+    // exchange rows and barriers by compile-time offsets (the row loop is unrolled by two)
+    const char *sp = reinterpret_cast<const char *>(ring) + sizeof(RowStage<T>) + tid * CPT * sizeof(T);   // slot 1
+    const char *op = reinterpret_cast<const char *>(&ring[1].occ[tid * CPT]);
+    uint64_t *tbar = &bars[1];
+    int slot = 1;
+    uint32_t tma_par = 0, xpar = 0;
+    T *my_st = &s.st[0][0][tid];
+    T *my_fx = &s.fx[0][0][tid];
+    constexpr int ST_B = 4 * NT, FX_B = 3 * NT;         // stride of the row-parity index of st / fx
+    const bool last_thread = tid == NT - 1, first_thread = tid == 0;
+    T *out_h = Ho + (size_t)y0 * nx + i, *out_qx = QXo + (size_t)y0 * nx + i, *out_qy = QYo + (size_t)y0 * nx + i;
+    const int nit = R + 1;                             // iteration it handles grid row y0 + it (ring row it + 1)
+
+    if constexpr (std::is_same<T, float>::value && CPT == 2) {
+    // ---- fp32: the two columns of a thread as one packed pair (flood_pk.cuh)
+    f2 eta_q = pk(eta_p[0], eta_p[1]), u_q = pk(u_p[0], u_p[1]), v_q = pk(v_p[0], v_p[1]), z_q = pk(z_p[0], z_p[1]);
+    f2 ah2 = pk1(0.f), ax2 = pk1(0.f), ay2 = pk1(0.f), n0_q = pk1(0.f);
+    int occ_q0 = 0, occ_q1 = 0;
+    const f2 dtdx2 = pk1(dtdx), dtdy2 = pk1(dtdy), ndtdy2 = pk1(-dtdy);
+
+    auto row = [&](auto qc, int it) {
+        constexpr int b = decltype(qc)::value;
+        mbar_wait(tbar, tma_par);
+        const RowStage<float> &st = *reinterpret_cast<const RowStage<float> *>(sp);
+        const f2 hc = *reinterpret_cast<const f2 *>(st.h), qxc = *reinterpret_cast<const f2 *>(st.qx);
+        const f2 qyc = *reinterpret_cast<const f2 *>(st.qy), z = *reinterpret_cast<const f2 *>(st.z);
+        const f2 n0_c = *reinterpret_cast<const f2 *>(st.n0);
+        const ByteN<2> occ_c = *reinterpret_cast<const ByteN<2> *>(op);
+        f2 eta, u, v;
+        prims_x2(hc, qxc, qyc, z, h_dry, eta, u, v);
+        float *stb = my_st + b * ST_B;
+        stb[0] = eta.y; stb[NT] = u.y; stb[2 * NT] = v.y; stb[3 * NT] = z.y;
+        mbar_arrive(&xbar[b]);                         // publishes st[b] of this row and fx[b^1] of the previous one
+
+        // south faces of the current row = north faces of the previous one (normal velocity v)
+        f2 g0, g1L, g1R, g2;
+        face_eta_x2(g, eta_q, v_q, u_q, z_q, eta, v, u, z, g0, g1L, g1R, g2);
+
+        mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
+        if (warp == 0 && it + 1 + STAGES < nrows) {
+            if (elect_one()) tm_issue_row(a, H, QX, QY, ring[slot], tbar, x0, y0 + it + STAGES);
+        }
+        sp += sizeof(RowStage<float>); op += sizeof(RowStage<float>); tbar += 1;
+        if (++slot == STAGES) {
+            slot = 0; tma_par ^= 1u;
+            sp -= STAGES * sizeof(RowStage<float>); op -= STAGES * sizeof(RowStage<float>); tbar -= STAGES;
+        }
+
+        if (it > 0) {                                  // finish row y0 + it - 1
+            const float *fe = last_thread ? &s.er[0][it - 1] : my_fx + (b ^ 1) * FX_B + 1;
+            const int stride = last_thread ? MARCH_MAX_R : NT;
+            const float e0 = fe[0], e1 = fe[stride], e2 = fe[2 * stride];
+            // a warp whose cells of this row hold exact zeros and receive no flux writes zeros
+            // (sign bits shifted out: -0 counts as zero)
+            unsigned bits = __float_as_uint(e0) | __float_as_uint(e1) | __float_as_uint(e2)
+                          | __float_as_uint(g0.x) | __float_as_uint(g0.y) | __float_as_uint(g1L.x) | __float_as_uint(g1L.y)
+                          | __float_as_uint(g2.x) | __float_as_uint(g2.y);
+            const bool live = live_p || (bits << 1) != 0u;
+            f2 ho = pk1(0.f), qxo = pk1(0.f), qyo = pk1(0.f);
+            if (__any_sync(0xffffffffu, live)) {
+                ho = fma2(ndtdy2, g0, ah2); qxo = fma2(ndtdy2, g2, ax2); qyo = fma2(ndtdy2, g1L, ay2);
+                ho.y = fmaf(-dtdx, e0, ho.y); qxo.y = fmaf(-dtdx, e1, qxo.y); qyo.y = fmaf(-dtdx, e2, qyo.y);
+                finish_hat_x2(a, dt, ho, qxo, qyo, n0_q, occ_q0, occ_q1, lam, clamp_h, clamp_n);
+            }
+            *reinterpret_cast<f2 *>(out_h) = ho;
+            *reinterpret_cast<f2 *>(out_qx) = qxo;
+            *reinterpret_cast<f2 *>(out_qy) = qyo;
+            out_h += nx; out_qx += nx; out_qy += nx;
+        }
+        if (it < R) {                                  // enter row y0 + it: west faces, start its accumulators
+            const float *sl = first_thread ? &s.sw[0][it] : stb - 1;
+            const int stride = first_thread ? MARCH_MAX_R : NT;
+            // face .x: (left neighbour | my column 0), face .y: (my column 0 | my column 1)
+            f2 f0, f1L, f1R, f2v;
+            face_eta_x2(g, pk(sl[0], eta.x), pk(sl[stride], u.x), pk(sl[2 * stride], v.x), pk(sl[3 * stride], z.x),
+                        eta, u, v, z, f0, f1L, f1R, f2v);
+            float *fxb = my_fx + b * FX_B;
+            fxb[0] = f0.x; fxb[NT] = f1L.x; fxb[2 * NT] = f2v.x;
+            ah2 = fma2(dtdx2, f0, fma2(dtdy2, g0, hc));
+            ax2 = fma2(dtdx2, f1R, fma2(dtdy2, g2, qxc));
+            ay2 = fma2(dtdx2, f2v, fma2(dtdy2, g1R, qyc));
+            // east face of column 0 = west face of column 1
+            ah2.x = fmaf(-dtdx, f0.y, ah2.x); ax2.x = fmaf(-dtdx, f1L.y, ax2.x); ay2.x = fmaf(-dtdx, f2v.y, ay2.x);
+            const unsigned ab = __float_as_uint(ah2.x) | __float_as_uint(ah2.y) | __float_as_uint(ax2.x)
+                              | __float_as_uint(ax2.y) | __float_as_uint(ay2.x) | __float_as_uint(ay2.y);
+            live_p = (ab << 1) != 0u;
+        }
+        eta_q = eta; u_q = u; v_q = v; z_q = z;
+        n0_q = n0_c; occ_q0 = a.couple ? (int)occ_c.v[0] : 0; occ_q1 = a.couple ? (int)occ_c.v[1] : 0;
+    };
+
+    for (int base = 0; base < nit; base += 2) {
+        row(std::integral_constant<int, 0>{}, base);
+        if (base + 1 < nit) row(std::integral_constant<int, 1>{}, base + 1);
+        xpar ^= 1u;
+    }
+    } else {
+    auto row = [&](auto qc, int it) {
+        constexpr int b = decltype(qc)::value;
+        mbar_wait(tbar, tma_par);
+        const RowStage<T> &st = *reinterpret_cast<const RowStage<T> *>(sp);
+        const VecN<T, CPT> hv = *reinterpret_cast<const VecN<T, CPT> *>(st.h);
+        const VecN<T, CPT> qxv = *reinterpret_cast<const VecN<T, CPT> *>(st.qx);
+        const VecN<T, CPT> qyv = *reinterpret_cast<const VecN<T, CPT> *>(st.qy);
+        const VecN<T, CPT> zv = *reinterpret_cast<const VecN<T, CPT> *>(st.z);
+        const VecN<T, CPT> n0_c = *reinterpret_cast<const VecN<T, CPT> *>(st.n0);
+        const ByteN<CPT> occ_c = *reinterpret_cast<const ByteN<CPT> *>(op);
         T eta[CPT], u[CPT], v[CPT], z[CPT], hc[CPT], qxc[CPT], qyc[CPT];
 #pragma unroll
         for (int k = 0; k < CPT; ++k) {
-            Raw4<T> q{hv.v[k], qxv.v[k], qyv.v[k], zv.v[k]};
-            march_prims<T, false>(q, h_dry, eta[k], u[k], v[k]);
-            z[k] = q.z; hc[k] = q.h; qxc[k] = q.qx; qyc[k] = q.qy;
+            Raw4<T> qq{hv.v[k], qxv.v[k], qyv.v[k], zv.v[k]};
+            march_prims<T, false>(qq, h_dry, eta[k], u[k], v[k]);
+            z[k] = qq.z; hc[k] = qq.h; qxc[k] = qq.qx; qyc[k] = qq.qy;
         }
-        const int b = jj & 1;
-        s.st[b][0][tid] = eta[CPT - 1]; s.st[b][1][tid] = u[CPT - 1];
-        s.st[b][2][tid] = v[CPT - 1];   s.st[b][3][tid] = z[CPT - 1];
+        T *stb = my_st + b * ST_B;
+        stb[0] = eta[CPT - 1]; stb[NT] = u[CPT - 1]; stb[2 * NT] = v[CPT - 1]; stb[3 * NT] = z[CPT - 1];
         mbar_arrive(&xbar[b]);                         // publishes st[b] of this row and fx[b^1] of the previous one
 
         // south faces of the current row = north faces of the previous one (normal velocity v)
@@ -191,16 +291,19 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         for (int k = 0; k < CPT; ++k)
             face_eta<T, false, true>(g, eta_p[k], v_p[k], u_p[k], z_p[k], eta[k], v[k], u[k], z[k], g0[k], g1L[k], g1R[k], g2[k]);
 
-        mbar_wait(&xbar[b], (uint32_t)((jj - y0) >> 1) & 1u);
-        if (warp == 0 && r + STAGES < nrows) {
-            if (elect_one()) tm_issue_row(a, H, QX, QY, ring[slot], &bars[slot], x0, y0 - 1 + r + STAGES);
+        mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
+        if (warp == 0 && it + 1 + STAGES < nrows) {
+            if (elect_one()) tm_issue_row(a, H, QX, QY, ring[slot], tbar, x0, y0 + it + STAGES);
         }
-        if (++slot == STAGES) { slot = 0; phase ^= 1u; }
+        sp += sizeof(RowStage<T>); op += sizeof(RowStage<T>); tbar += 1;
+        if (++slot == STAGES) {
+            slot = 0; tma_par ^= 1u;
+            sp -= STAGES * sizeof(RowStage<T>); op -= STAGES * sizeof(RowStage<T>); tbar -= STAGES;
+        }
 
-        if (jj > y0) {                                 // finish row jj-1
-            const int j = jj - 1, bp = b ^ 1;
-            const T *fe = (tid == NT - 1) ? &s.er[0][j - y0] : &s.fx[bp][0][tid + 1];
-            const int stride = (tid == NT - 1) ? MARCH_MAX_R : NT;
+        if (it > 0) {                                  // finish row y0 + it - 1
+            const T *fe = last_thread ? &s.er[0][it - 1] : my_fx + (b ^ 1) * FX_B + 1;
+            const int stride = last_thread ? MARCH_MAX_R : NT;
             const T e0 = fe[0], e1 = fe[stride], e2 = fe[2 * stride];
             // a warp whose cells of this row hold exact zeros and receive no flux writes zeros
             bool live = live_p || e0 != T(0) || e1 != T(0) || e2 != T(0);
@@ -218,14 +321,14 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                     ho.v[k] = hn; qxo.v[k] = qxn; qyo.v[k] = qyn;
                 }
             }
-            const size_t c = (size_t)j * nx + i;
-            *reinterpret_cast<VecN<T, CPT> *>(Ho + c) = ho;
-            *reinterpret_cast<VecN<T, CPT> *>(QXo + c) = qxo;
-            *reinterpret_cast<VecN<T, CPT> *>(QYo + c) = qyo;
+            *reinterpret_cast<VecN<T, CPT> *>(out_h) = ho;
+            *reinterpret_cast<VecN<T, CPT> *>(out_qx) = qxo;
+            *reinterpret_cast<VecN<T, CPT> *>(out_qy) = qyo;
+            out_h += nx; out_qx += nx; out_qy += nx;
         }
-        if (jj < y1) {                                 // enter row jj: west faces, start its accumulators
-            const T *sl = (tid == 0) ? &s.sw[0][jj - y0] : &s.st[b][0][tid - 1];
-            const int stride = (tid == 0) ? MARCH_MAX_R : NT;
+        if (it < R) {                                  // enter row y0 + it: west faces, start its accumulators
+            const T *sl = first_thread ? &s.sw[0][it] : stb - 1;
+            const int stride = first_thread ? MARCH_MAX_R : NT;
             T f0[CPT], f1L[CPT], f1R[CPT], f2[CPT];
             face_eta<T, false, true>(g, sl[0], sl[stride], sl[2 * stride], sl[3 * stride], eta[0], u[0], v[0], z[0],
                                      f0[0], f1L[0], f1R[0], f2[0]);
@@ -233,7 +336,8 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
             for (int k = 1; k < CPT; ++k)
                 face_eta<T, false, true>(g, eta[k - 1], u[k - 1], v[k - 1], z[k - 1], eta[k], u[k], v[k], z[k],
                                          f0[k], f1L[k], f1R[k], f2[k]);
-            s.fx[b][0][tid] = f0[0]; s.fx[b][1][tid] = f1L[0]; s.fx[b][2][tid] = f2[0];
+            T *fxb = my_fx + b * FX_B;
+            fxb[0] = f0[0]; fxb[NT] = f1L[0]; fxb[2 * NT] = f2[0];
             live_p = false;
 #pragma unroll
             for (int k = 0; k < CPT; ++k) {
@@ -249,6 +353,13 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
             eta_p[k] = eta[k]; u_p[k] = u[k]; v_p[k] = v[k]; z_p[k] = z[k];
             n0_p[k] = n0_c.v[k]; occ_p[k] = a.couple ? (int)occ_c.v[k] : 0;
         }
+    };
+
+    for (int base = 0; base < nit; base += 2) {
+        row(std::integral_constant<int, 0>{}, base);
+        if (base + 1 < nit) row(std::integral_constant<int, 1>{}, base + 1);
+        xpar ^= 1u;
+    }
     }
     if (clamp_n) {
         atomicAdd(&a.ctl->clamped_volume, (double)clamp_h * (double)a.cell_area);

@@ -259,7 +259,7 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
     FloodArgs<T> fa = flood_args<T>(s);
     mark();
     if (s->flood_variant == 4) {
-        launch_tmarch<T, 2, 5, 5>(fa, dim3(s->march_gx, s->march_gy), st);
+        launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st);
     } else if (s->flood_variant == 3) {
         flood_march2_kernel<T, 2><<<dim3(s->march_gx, s->march_gy), MW / 2, 0, st>>>(fa);
     } else if (s->flood_variant == 2) {
