@@ -154,6 +154,8 @@ def run_ours(args):
         g.set_flood_variant(args.flood_variant)
     if args.no_overlap:
         g.set_overlap(False)
+    if args.march_rows > 0:
+        g.set_march_rows(args.march_rows)
     variant = g.flood_variant()
     kps = g.kernels_per_step()
 
@@ -289,6 +291,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--flood-variant", type=int, default=-1, choices=list(range(-1, 5)), help="-1: the library default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--march-rows", type=int, default=0, help="rows per chunk of the row-marching flood kernel (0: library default)")
     ap.add_argument("--no-overlap", action="store_true", help="pedestrian step and flood step in one chain instead of parallel graph branches")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -25,6 +25,7 @@ struct Ctl {
     int cursor, layer, bags, complete;
     unsigned int scan_epoch;         // makes the look-back flags of the scan self-resetting
     unsigned int scan_ticket;        // dynamic tile index of the scan
+    int occ_next;                    // N_p buffer the binning chain of the NEXT step fills (= parity ^ 1), published by the pedestrian step
 };
 
 template <typename T> struct Vec4 { T v[4]; };

@@ -28,7 +28,8 @@ struct FloodArgs {
     T *h[2], *qx[2], *qy[2];          // ping-pong conserved state, SoA, row-major
     const T *zs;                      // bed elevation; +inf marks a solid cell
     const T *n0;                      // initial Manning n_M per cell
-    const uint8_t *occ;               // N_p per cell of the current step (saturated at 255)
+    const uint8_t *occ;               // N_p per cell (saturated at 255): buffer 0; the step at flood parity p reads occ + p * occ_stride
+    size_t occ_stride;
     const uint8_t *inflow[4];         // per edge cell: number of inflow faces on that side (W,E,S,N)
     const uint8_t *chunk_flag;        // march kernel: 1 = chunk takes the general path (flood_march.cuh)
     int R;                            // march kernel: rows per chunk
@@ -143,6 +144,7 @@ __global__ void __launch_bounds__(256) flood_cell_kernel(FloodArgs<T> a)
     __shared__ T red[32];
     if (a.ctl->halt) return;
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
     const T *__restrict__ Z = a.zs;
     const T dt = (T)a.ctl->dt, qin = (T)a.ctl->q_in;
@@ -178,7 +180,7 @@ __global__ void __launch_bounds__(256) flood_cell_kernel(FloodArgs<T> a)
             if (j == 0) GS0 += qin * T(a.inflow[2][i]);
             if (j == a.ny - 1) GN0 -= qin * T(a.inflow[3][i]);
             finish_cell(a, dt, h, qx, qy, FE0 - FW0, FE1 - FW1, FE2 - FW2, GN0 - GS0, GN1 - GS1, GN2 - GS2,
-                        a.n0[c], (int)a.occ[c], hn, qxn, qyn, lam);
+                        a.n0[c], (int)OCC[c], hn, qxn, qyn, lam);
         }
         a.h[p ^ 1][c] = hn; a.qx[p ^ 1][c] = qxn; a.qy[p ^ 1][c] = qyn;
     }
@@ -213,6 +215,7 @@ __global__ void __launch_bounds__(FLOOD_TILE_THREADS, sizeof(T) == 4 ? 3 : 1) fl
     TileSmem<T> &s = *reinterpret_cast<TileSmem<T> *>(smem_raw);
     if (a.ctl->halt) return;
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
     const T *__restrict__ Z = a.zs;
     const T dt = (T)a.ctl->dt, qin = (T)a.ctl->q_in;
@@ -325,7 +328,7 @@ __global__ void __launch_bounds__(FLOOD_TILE_THREADS, sizeof(T) == 4 ? 3 : 1) fl
     if (inside) {
         const size_t c = (size_t)gy * a.nx + gx;
         const Vec4<T> n4 = *reinterpret_cast<const Vec4<T> *>(a.n0 + c);
-        const uchar4 o4 = *reinterpret_cast<const uchar4 *>(a.occ + c);
+        const uchar4 o4 = *reinterpret_cast<const uchar4 *>(OCC + c);
         const int occ[4] = {o4.x, o4.y, o4.z, o4.w};
         const T fe0 = s.xfl[0][ty][tx + 1], fe1L = s.xfl[1][ty][tx + 1], fe2 = s.xfl[2][ty][tx + 1];
         const Vec4<T> n0v = *reinterpret_cast<const Vec4<T> *>(&s.yfl[0][ty + 1][4 * tx]);
@@ -373,6 +376,7 @@ __global__ void flood_lambda_kernel(FloodArgs<T> a)
 {
     __shared__ T red[32];
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     T lam = T(0);
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < (size_t)a.nx * a.ny;
          c += (size_t)gridDim.x * blockDim.x) {
@@ -390,6 +394,7 @@ template <typename T>
 __global__ void flood_derive_kernel(FloodArgs<T> a, T *u, T *v, T *hr)
 {
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < (size_t)a.nx * a.ny;
          c += (size_t)gridDim.x * blockDim.x) {
         const T h = a.h[p][c];
@@ -410,6 +415,7 @@ __global__ void flood_stats_kernel(FloodArgs<T> a, double *out /* volume, max_h,
 {
     __shared__ double sv[32], sh[32], sr[32], sb[32];
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     double vol = 0, mh = 0, mr = 0, bad = 0;
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < (size_t)a.nx * a.ny;
          c += (size_t)gridDim.x * blockDim.x) {

@@ -124,6 +124,7 @@ __device__ __forceinline__ T march_chunk(const FloodArgs<T> &a, MarchSmem<T> &s,
     const int tid = threadIdx.x;
     const int nx = a.nx, ny = a.ny;
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
     const T *__restrict__ Z = a.zs;
     T *__restrict__ Ho = a.h[p ^ 1], *__restrict__ QXo = a.qx[p ^ 1], *__restrict__ QYo = a.qy[p ^ 1];
@@ -181,7 +182,7 @@ __device__ __forceinline__ T march_chunk(const FloodArgs<T> &a, MarchSmem<T> &s,
         if (jj < y1 && col_ok) {
             const size_t c = (size_t)jj * nx + i;
             n0_c = a.n0[c];
-            occ_c = a.couple ? (int)a.occ[c] : 0;
+            occ_c = a.couple ? (int)OCC[c] : 0;
         }
         __syncthreads();
 

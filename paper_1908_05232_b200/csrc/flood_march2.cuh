@@ -78,6 +78,7 @@ __device__ __forceinline__ T march2_chunk(const FloodArgs<T> &a, March2Smem<T, C
     const int tid = threadIdx.x;
     const int nx = a.nx, ny = a.ny;
     const int p = a.ctl->parity;
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
     const T *__restrict__ Z = a.zs;
     T *__restrict__ Ho = a.h[p ^ 1], *__restrict__ QXo = a.qx[p ^ 1], *__restrict__ QYo = a.qy[p ^ 1];
@@ -150,7 +151,7 @@ __device__ __forceinline__ T march2_chunk(const FloodArgs<T> &a, March2Smem<T, C
         if (jj < y1 && col_ok) {
             const size_t c = (size_t)jj * nx + i;
             n0_c = *reinterpret_cast<const VecN<T, CPT> *>(a.n0 + c);
-            if (a.couple) occ_c = *reinterpret_cast<const ByteN<CPT> *>(a.occ + c);
+            if (a.couple) occ_c = *reinterpret_cast<const ByteN<CPT> *>(OCC + c);
         }
         __syncthreads();
 

@@ -23,6 +23,10 @@
 
 namespace fp {
 
+#ifndef TM_SPLIT_BARRIER
+#define TM_SPLIT_BARRIER 0
+#endif
+
 template <typename T>
 struct __align__(16) RowStage {
     T h[MW], qx[MW], qy[MW], z[MW], n0[MW];
@@ -68,7 +72,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 // one row segment (columns x0 .. x0+MW-1 of row j) -> stage
 template <typename T>
-__device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, const T *QX, const T *QY,
+__device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, const T *QX, const T *QY, const uint8_t *OCC,
                                              RowStage<T> &st, uint64_t *bar, int x0, int j)
 {
     const size_t c = (size_t)j * a.nx + x0;
@@ -79,7 +83,7 @@ __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, 
     bulk_g2s(st.qy, QY + c, RB, bar);
     bulk_g2s(st.z, a.zs + c, RB, bar);
     bulk_g2s(st.n0, a.n0 + c, RB, bar);
-    bulk_g2s(st.occ, a.occ + c, MW, bar);
+    bulk_g2s(st.occ, OCC + c, MW, bar);
 }
 
 // interior chunk (no domain edge, no solid cell in it or in its halo): rows y0-1 .. y0+R all exist
@@ -100,6 +104,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);       // warp-uniform by construction
     const int nx = a.nx;
     const int p = __shfl_sync(0xffffffffu, a.ctl->parity, 0);
+    const uint8_t *__restrict__ OCC = a.occ + (size_t)p * a.occ_stride;
     const T *__restrict__ H = a.h[p], *__restrict__ QX = a.qx[p], *__restrict__ QY = a.qy[p];
     const T *__restrict__ Z = a.zs;
     T *__restrict__ Ho = a.h[p ^ 1], *__restrict__ QXo = a.qx[p ^ 1], *__restrict__ QYo = a.qy[p ^ 1];
@@ -119,7 +124,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     __syncthreads();
     if (warp == 0) {
         if (elect_one())
-            for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row(a, H, QX, QY, ring[r], &bars[r], x0, y0 - 1 + r);
+            for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row(a, H, QX, QY, OCC, ring[r], &bars[r], x0, y0 - 1 + r);
     }
 
     // ---- pre-pass: strip-edge data for every row of the chunk (as in variants 2, 3)
@@ -155,7 +160,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     }
     __syncthreads();                                   // slot 0 consumed; er/sw visible
     if (warp == 0 && STAGES < nrows) {
-        if (elect_one()) tm_issue_row(a, H, QX, QY, ring[0], &bars[0], x0, y0 - 1 + STAGES);
+        if (elect_one()) tm_issue_row(a, H, QX, QY, OCC, ring[0], &bars[0], x0, y0 - 1 + STAGES);
     }
 
     T ah[CPT], ax[CPT], ay[CPT], n0_p[CPT];
@@ -199,15 +204,21 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         prims_x2(hc, qxc, qyc, z, h_dry, eta, u, v);
         float *stb = my_st + b * ST_B;
         stb[0] = eta.y; stb[NT] = u.y; stb[2 * NT] = v.y; stb[3 * NT] = z.y;
+#if TM_SPLIT_BARRIER
         mbar_arrive(&xbar[b]);                         // publishes st[b] of this row and fx[b^1] of the previous one
+#endif
 
         // south faces of the current row = north faces of the previous one (normal velocity v)
         f2 g0, g1L, g1R, g2;
         face_eta_x2(g, eta_q, v_q, u_q, z_q, eta, v, u, z, g0, g1L, g1R, g2);
 
+#if TM_SPLIT_BARRIER
         mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
+#else
+        __syncthreads();                               // st[b] of this row and fx[b^1] of the previous one are visible
+#endif
         if (warp == 0 && it + 1 + STAGES < nrows) {
-            if (elect_one()) tm_issue_row(a, H, QX, QY, ring[slot], tbar, x0, y0 + it + STAGES);
+            if (elect_one()) tm_issue_row(a, H, QX, QY, OCC, ring[slot], tbar, x0, y0 + it + STAGES);
         }
         sp += sizeof(RowStage<float>); op += sizeof(RowStage<float>); tbar += 1;
         if (++slot == STAGES) {
@@ -283,7 +294,9 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         }
         T *stb = my_st + b * ST_B;
         stb[0] = eta[CPT - 1]; stb[NT] = u[CPT - 1]; stb[2 * NT] = v[CPT - 1]; stb[3 * NT] = z[CPT - 1];
+#if TM_SPLIT_BARRIER
         mbar_arrive(&xbar[b]);                         // publishes st[b] of this row and fx[b^1] of the previous one
+#endif
 
         // south faces of the current row = north faces of the previous one (normal velocity v)
         T g0[CPT], g1L[CPT], g1R[CPT], g2[CPT];
@@ -291,9 +304,13 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         for (int k = 0; k < CPT; ++k)
             face_eta<T, false, true>(g, eta_p[k], v_p[k], u_p[k], z_p[k], eta[k], v[k], u[k], z[k], g0[k], g1L[k], g1R[k], g2[k]);
 
+#if TM_SPLIT_BARRIER
         mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
+#else
+        __syncthreads();                               // st[b] of this row and fx[b^1] of the previous one are visible
+#endif
         if (warp == 0 && it + 1 + STAGES < nrows) {
-            if (elect_one()) tm_issue_row(a, H, QX, QY, ring[slot], tbar, x0, y0 + it + STAGES);
+            if (elect_one()) tm_issue_row(a, H, QX, QY, OCC, ring[slot], tbar, x0, y0 + it + STAGES);
         }
         sp += sizeof(RowStage<T>); op += sizeof(RowStage<T>); tbar += 1;
         if (++slot == STAGES) {

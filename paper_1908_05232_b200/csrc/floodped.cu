@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -65,8 +66,9 @@ struct sim {
     int exit_i[16]{}, exit_j[16]{};
     cudaGraphExec_t graph1 = nullptr, graphN = nullptr;
     cudaStream_t stream2 = nullptr;   // second branch of the step graph (pedestrian step beside the flood step)
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_ped = nullptr, ev_occ = nullptr, ev_tail = nullptr;
     int overlap = 1;
+    bool binned = false;             // the binning chain of the upcoming step has run on the current state
     std::string err;
 };
 
@@ -98,7 +100,7 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 2; ++k) { s->h[k] = real(nc); s->qx[k] = real(nc); s->qy[k] = real(nc); }
     s->zs = real(nc); s->z0 = real(nc); s->n0 = real(nc);
     for (int k = 0; k < 3; ++k) s->scratch_real[k] = real(nc);
-    s->occ = b.take<uint8_t>(nc); s->mask = b.take<uint8_t>(nc);
+    s->occ = b.take<uint8_t>(2 * nc); s->mask = b.take<uint8_t>(nc);
     s->inflow[0] = b.take<uint8_t>(s->grid.ny); s->inflow[1] = b.take<uint8_t>(s->grid.ny);
     s->inflow[2] = b.take<uint8_t>(s->grid.nx); s->inflow[3] = b.take<uint8_t>(s->grid.nx);
     s->nav = b.take<uint8_t>((size_t)s->n_targets * nc);
@@ -114,7 +116,7 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 5; ++k) s->ped_out[k] = real(np);
     for (int k = 0; k < 3; ++k) s->ped_out_u8[k] = b.take<uint8_t>(np);
     for (int k = 0; k < 2; ++k) s->ped_out_i32[k] = b.take<int32_t>(np);
-    s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(np);
+    s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(2 * np);
     s->bxy = real(2 * (size_t)np);
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
     s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * ((s->grid.ny + 7) / 8));    // room for any R >= 8
@@ -142,8 +144,9 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     // march kernel geometry: strips of MW columns, chunks of R rows; R shrinks until the grid
     // fills the 148 SMs a few times over
     s->march_gx = (g->nx + MW - 1) / MW;
-    // about 12 waves of 148 SMs x 5 resident CTAs (measured best on 8192^2: R = 24..32)
-    s->march_R = (int)(((long long)g->ny * s->march_gx) / (12 * 148 * 5));
+    // about 15 waves of 148 SMs x 6 resident CTAs (measured on 8192^2: flat optimum R = 14..24;
+    // short chunks even out the dry/wet imbalance between CTAs, halo rows cost little: not DRAM-bound)
+    s->march_R = (int)(((long long)g->ny * s->march_gx) / (15 * 148 * 6));
     if (s->march_R > MARCH_MAX_R) s->march_R = MARCH_MAX_R;
     if (s->march_R < 16) s->march_R = 16;
     s->march_gy = (g->ny + s->march_R - 1) / s->march_R;
@@ -168,7 +171,7 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     a.h_dry = (T)s->prm.h_dry; a.cell_area = (T)(s->grid.dx * s->grid.dy);
     a.couple = s->prm.couple_roughness; a.n_cap = s->prm.n_cap;
     for (int k = 0; k < 2; ++k) { a.h[k] = (T *)s->h[k]; a.qx[k] = (T *)s->qx[k]; a.qy[k] = (T *)s->qy[k]; }
-    a.zs = (const T *)s->zs; a.n0 = (const T *)s->n0; a.occ = s->occ;
+    a.zs = (const T *)s->zs; a.n0 = (const T *)s->n0; a.occ = s->occ; a.occ_stride = (size_t)s->ncell;
     for (int k = 0; k < 4; ++k) a.inflow[k] = s->inflow[k];
     a.chunk_flag = s->chunk_flag; a.R = s->march_R;
     a.ctl = s->ctl;
@@ -205,6 +208,7 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
     a.A = ped_soa<T>(s, 0); a.B = ped_soa<T>(s, 1);
     a.key = s->key; a.off = s->off; a.count = s->count; a.start = s->start; a.cellprev = s->cellprev;
     a.occ = s->occ; a.mask = s->mask; a.nav = s->nav;
+    a.occ_stride = (size_t)s->ncell; a.cellprev_stride = (size_t)s->np; a.pipelined = 0;
     a.bxy = (VecN<T, 2> *)s->bxy;
     a.c_exp1 = (T)(2.0 * p.radius / p.B_s * 1.4426950408889634 + std::log2(p.A_s));   // A e^{(2r-d)/B} = 2^{c1 + c2 d}
     a.c_exp2 = (T)(-1.4426950408889634 / p.B_s);
@@ -224,40 +228,44 @@ template <typename T> TailArgs<T> tail_args(const sim *s)
     return a;
 }
 
-// ---- enqueue the kernels of ONE coupled step on `st` (same arguments every step: the
-// ping-pong parity, dt, t, halt live in the device control block)
-template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev = nullptr)
+// ---- launch helpers.  Kernel arguments are the same every step: the ping-pong parity, dt, t,
+// halt live in the device control block.
+template <typename T> PedArgs<T> ped_args_full(const sim *s, int pipelined)
 {
     PedArgs<T> pa = ped_args<T>(s);
     for (int e = 0; e < s->prm.n_exit_cells; ++e) { pa.exit_i[e] = s->exit_i[e]; pa.exit_j[e] = s->exit_j[e]; }
     pa.n_exit = s->prm.n_exit_cells;
-    int k = 0;
-    auto mark = [&]() { if (ev) cudaEventRecord(ev[k++], st); };     // profiling mode only
-    // flood and pedestrian step both read level n only: in graph mode they run as parallel branches
-    const bool fork = !ev && s->np > 0 && s->overlap;
-    if (s->np > 0) {
-        const int nb = (s->np + 255) / 256;
-        mark();
-        ped_bin_count_kernel<T><<<nb, 256, 0, st>>>(pa, 1);
-        const int n_items = s->nbins + 1;
-        mark();
-        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, st>>>(s->count, s->start, n_items, s->scan_status, s->ctl);
-        mark();
-        ped_scatter_kernel<T><<<nb, 256, 0, st>>>(pa);
-        mark();
-        ped_occ_kernel<T><<<nb, 256, 0, st>>>(pa);
-        mark();
-        if (fork) {
-            CU(cudaEventRecord(s->ev_fork, st));
-            CU(cudaStreamWaitEvent(s->stream2, s->ev_fork, 0));
-            ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, s->stream2>>>(pa);
-            CU(cudaEventRecord(s->ev_join, s->stream2));
-        } else {
-            ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, st>>>(pa);
-        }
-    } else k = 5;
-    FloodArgs<T> fa = flood_args<T>(s);
+    pa.pipelined = pipelined;
+    return pa;
+}
+
+struct Marks {                                        // profiling mode only: an event before each launch
+    cudaEvent_t *ev; int k; cudaStream_t st;
+    void operator()() { if (ev) cudaEventRecord(ev[k++], st); }
+};
+
+// (B)+(O) of the step that comes NEXT: count -> scan -> scatter -> N_p per cell.  It needs the
+// pedestrians of that step only, so in graph mode it runs beside the flood kernel of the step
+// before (pipelined = 1: it fills the N_p buffer the flood kernel is not reading).
+template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelined, Marks &mark)
+{
+    PedArgs<T> pa = ped_args_full<T>(s, pipelined);
+    const int nb = (s->np + 255) / 256, n_items = s->nbins + 1;
     mark();
+    ped_bin_count_kernel<T><<<nb, 256, 0, st>>>(pa, 1);
+    mark();
+    scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, st>>>(s->count, s->start, n_items, s->scan_status, s->ctl, pipelined);
+    mark();
+    ped_scatter_kernel<T><<<nb, 256, 0, st>>>(pa);
+    mark();
+    ped_occ_kernel<T><<<nb, 256, 0, st>>>(pa);
+    CU(cudaGetLastError());
+    return SIM_OK;
+}
+
+template <typename T> void launch_flood(sim *s, cudaStream_t st)
+{
+    FloodArgs<T> fa = flood_args<T>(s);
     if (s->flood_variant == 4) {
         launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st);
     } else if (s->flood_variant == 3) {
@@ -271,11 +279,61 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
         dim3 blk(32, 8), grid((s->grid.nx + 31) / 32, (s->grid.ny + 7) / 8);
         flood_cell_kernel<T><<<grid, blk, 0, st>>>(fa);
     }
+}
+
+// ONE coupled step n on `st`, given that the binning chain of step n has run (sim::binned):
+//     pedestrian step n | flood step n  ->  tail n ;   binning chain of step n+1
+// Every read of step n is at level n, so the pedestrian step and the flood step are independent;
+// the binning chain of step n+1 needs the pedestrian step n only.  In graph mode (fork) the
+// pedestrian kernels form a second branch: ped_step(n) -> chain(n+1) beside flood(n); tail(n)
+// joins flood(n) and ped_step(n) (deposits), flood(n+1) joins tail(n) and chain(n+1).
+template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cudaEvent_t *ev = nullptr)
+{
+    Marks mark{ev, 0, st};
+    const bool peds = s->np > 0;
+    const bool fork = !ev && peds && s->overlap;
+    cudaStream_t sp = fork ? s->stream2 : st;
+    if (peds) {
+        if (fork) {
+            if (first) { CU(cudaEventRecord(s->ev_fork, st)); CU(cudaStreamWaitEvent(sp, s->ev_fork, 0)); }
+            else CU(cudaStreamWaitEvent(sp, s->ev_tail, 0));
+        }
+        mark();
+        ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, sp>>>(ped_args_full<T>(s, 0));
+        if (fork) {
+            CU(cudaEventRecord(s->ev_ped, sp));
+            if (!first) CU(cudaStreamWaitEvent(st, s->ev_occ, 0));     // N_p of this step, filled beside the step before
+        }
+    } else mark.k = 1;
     mark();
-    if (fork) CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+    launch_flood<T>(s, st);
+    if (fork) {
+        int rc = enqueue_bin_chain<T>(s, sp, 1, mark);
+        if (rc != SIM_OK) return rc;
+        CU(cudaEventRecord(s->ev_occ, sp));
+        CU(cudaStreamWaitEvent(st, s->ev_ped, 0));
+    }
+    mark();
     tail_kernel<T><<<1, 32, 0, st>>>(tail_args<T>(s), 0);
+    if (fork) CU(cudaEventRecord(s->ev_tail, st));
+    if (peds && !fork) {
+        int rc = enqueue_bin_chain<T>(s, st, 0, mark);               // after the tail: ctl->parity is that of step n+1
+        if (rc != SIM_OK) return rc;
+    }
     mark();
     CU(cudaGetLastError());
+    return SIM_OK;
+}
+
+// the binning chain of the upcoming step, when nothing has prepared it (first step, state re-injected)
+template <typename T> int prepare_bins(sim *s)
+{
+    if (s->np > 0 && !s->binned) {
+        Marks none{nullptr, 0, s->stream};
+        int rc = enqueue_bin_chain<T>(s, s->stream, 0, none);
+        if (rc != SIM_OK) return rc;
+    }
+    s->binned = true;
     return SIM_OK;
 }
 
@@ -283,20 +341,20 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, cudaEvent_t *ev 
 template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
 {
     constexpr int NE = 8, BATCH = 64;
-    static const int slot_of[NE - 1] = {0, 1, 2, 6, 3, 4, 5};       // launch order -> kernel_ms index
+    static const int slot_of[NE - 1] = {3, 4, 5, 0, 1, 2, 6};       // launch order -> kernel_ms index
     std::vector<cudaEvent_t> ev(NE * BATCH);
     for (auto &e : ev) CU(cudaEventCreate(&e));
     for (int k = 0; k < 8; ++k) ms[k] = 0.0;
-    int rc = SIM_OK;
+    int rc = prepare_bins<T>(s);
     while (n > 0 && rc == SIM_OK) {
         const int m = (int)(n < BATCH ? n : BATCH);
-        for (int i = 0; i < m && rc == SIM_OK; ++i) rc = enqueue_step<T>(s, s->stream, &ev[(size_t)i * NE]);
+        for (int i = 0; i < m && rc == SIM_OK; ++i) rc = enqueue_step<T>(s, s->stream, false, &ev[(size_t)i * NE]);
         if (rc != SIM_OK) break;
         cudaError_t e = cudaStreamSynchronize(s->stream);
         if (e != cudaSuccess) { rc = fail(s, SIM_ECUDA, cudaGetErrorString(e)); break; }
-        const int first = s->np > 0 ? 0 : 5;
+        const int first = s->np > 0 ? 0 : 1, last = s->np > 0 ? NE - 1 : 3;
         for (int i = 0; i < m; ++i)
-            for (int k = first; k < NE - 1; ++k) {
+            for (int k = first; k < last; ++k) {
                 float t = 0.f;
                 cudaEventElapsedTime(&t, ev[(size_t)i * NE + k], ev[(size_t)i * NE + k + 1]);
                 ms[slot_of[k]] += t;
@@ -321,7 +379,9 @@ template <typename T> int build_graphs(sim *s)
         cudaGraph_t g = nullptr;
         CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
         int rc = SIM_OK;
-        for (int r = 0; r < reps && rc == SIM_OK; ++r) rc = enqueue_step<T>(s, s->cap_stream);
+        for (int r = 0; r < reps && rc == SIM_OK; ++r) rc = enqueue_step<T>(s, s->cap_stream, r == 0);
+        if (rc == SIM_OK && s->np > 0 && s->overlap && cudaStreamWaitEvent(s->cap_stream, s->ev_occ, 0) != cudaSuccess)
+            rc = fail(s, SIM_ECUDA, "graph capture: join");
         cudaError_t e = cudaStreamEndCapture(s->cap_stream, &g);
         if (rc != SIM_OK) { if (g) cudaGraphDestroy(g); return rc; }
         if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
@@ -431,7 +491,8 @@ int upload_state(sim *s, const sim_topo_t *topo, const void *manning, const sim_
             id[i] = (int32_t)i;
         }
         if (upload(s, s->P[0].fsm, fsm.data(), np) || upload(s, s->P[0].active, act.data(), np) ||
-            upload(s, s->P[0].id, id.data(), np * 4) || upload(s, s->cellprev, neg.data(), np * 4))
+            upload(s, s->P[0].id, id.data(), np * 4) || upload(s, s->cellprev, neg.data(), np * 4) ||
+            upload(s, s->cellprev + np, neg.data(), np * 4))
             return SIM_ECUDA;
         CU(cudaStreamSynchronize(s->stream));
     }
@@ -529,9 +590,17 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     auto run = [&]() -> int {
         CU(cudaMemsetAsync(s->ws, 0, s->ws_bytes, s->stream));
         CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
-        CU(cudaStreamCreateWithFlags(&s->stream2, cudaStreamNonBlocking));
+        {   // the pedestrian branch of the step graph gets the SMs first: its small kernels then hide
+            // behind the flood kernel instead of queueing after its ~15 waves of CTAs
+            int lo = 0, hi = 0;
+            CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            const char *e = getenv("FLOODPED_PRIO");
+            CU(cudaStreamCreateWithPriority(&s->stream2, cudaStreamNonBlocking, (e && atoi(e) == 0) ? lo : hi));
+        }
         CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s->ev_ped, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s->ev_occ, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s->ev_tail, cudaEventDisableTiming));
         int r = DISPATCH(s, upload_state, s, topo, manning, peds, p);
         if (r != SIM_OK) return r;
         for (int k = 0; k < 4; ++k) if (upload(s, s->inflow[k], infl[k].data(), infl[k].size())) return SIM_ECUDA;
@@ -562,8 +631,13 @@ extern "C" int sim_step(sim_t *s, int64_t n)
 {
     if (!s) return SIM_EINVAL;
     if (n < 0) return fail(s, SIM_EINVAL, "negative step count");
+    if (n == 0) return SIM_OK;
     if (!s->graph1) {
         int rc = DISPATCH(s, build_graphs, s);
+        if (rc != SIM_OK) return rc;
+    }
+    {
+        int rc = DISPATCH(s, prepare_bins, s);
         if (rc != SIM_OK) return rc;
     }
     while (n >= GRAPH_CHUNK) { CU(cudaGraphLaunch(s->graphN, s->stream)); n -= GRAPH_CHUNK; }
@@ -707,16 +781,17 @@ template <typename T> int bin_peds_t(sim *s, int32_t *key, int32_t *order, int32
         const int halt = c.halt;
         if (halt) { c.halt = 0; CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream)); }
         ped_bin_count_kernel<T><<<nb, 256, 0, s->stream>>>(pa, 0);
-        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl);
+        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl, 0);
         ped_scatter_kernel<T><<<nb, 256, 0, s->stream>>>(pa);
         ped_key_by_id_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 0), s->key, np, s->ped_out_i32[0]);
         ped_gather_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 1), np, s->grid.nx, (T)1, (T)1, s->grid.ny,
             nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, s->ped_out_i32[1]);
         CU(cudaGetLastError());
-        // the scan consumed a ticket range and an epoch: re-arm them without touching dt
+        // (the scatter kernel has re-armed the scan)
         CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
         CU(cudaStreamSynchronize(s->stream));
-        c.scan_ticket = 0; c.scan_epoch += 1; c.halt = halt;
+        c.halt = halt;
+        s->binned = false;
         CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         if (copy_out(s, key, s->ped_out_i32[0], (size_t)np * 4) || copy_out(s, order, s->ped_out_i32[1], (size_t)np * 4))
             return SIM_ECUDA;
@@ -774,7 +849,11 @@ extern "C" int sim_read_conserved(sim_t *s, void *h, void *qx, void *qy)
 extern "C" int sim_read_occupancy(sim_t *s, uint8_t *np_cell)
 {
     if (!s) return SIM_EINVAL;
-    if (copy_out(s, np_cell, s->occ, (size_t)s->ncell)) return SIM_ECUDA;
+    Ctl c;
+    CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    // the most recent step ran at flood parity c.parity ^ 1 and read that N_p buffer
+    if (copy_out(s, np_cell, s->occ + (size_t)(c.parity ^ 1) * s->ncell, (size_t)s->ncell)) return SIM_ECUDA;
     CU(cudaStreamSynchronize(s->stream));
     return SIM_OK;
 }
@@ -807,6 +886,7 @@ extern "C" int sim_bin_peds(sim_t *s, int32_t *key, int32_t *order, int32_t *sta
 extern "C" int sim_write_flood(sim_t *s, const void *h, const void *qx, const void *qy, const void *z)
 {
     if (!s) return SIM_EINVAL;
+    s->binned = false;
     return DISPATCH(s, write_flood_t, s, h, qx, qy, z);
 }
 
@@ -814,6 +894,7 @@ extern "C" int sim_write_peds(sim_t *s, const void *x, const void *y, const void
                               const uint8_t *fsm, const uint8_t *active, const void *timer)
 {
     if (!s) return SIM_EINVAL;
+    s->binned = false;
     const size_t np = (size_t)s->np, rb = np * real_size(s);
     if (!np) return SIM_OK;
     // put buffer A back into original order first, so that index i means agent i again
@@ -846,8 +927,8 @@ extern "C" int sim_write_peds(sim_t *s, const void *x, const void *y, const void
     CU(cudaMemcpyAsync(s->P[0].role, role2.data(), np, cudaMemcpyHostToDevice, s->stream));
     CU(cudaMemcpyAsync(s->P[0].id, id.data(), np * 4, cudaMemcpyHostToDevice, s->stream));
     // occupancy bookkeeping restarts from scratch
-    CU(cudaMemsetAsync(s->occ, 0, (size_t)s->ncell, s->stream));
-    CU(cudaMemsetAsync(s->cellprev, 0xff, np * 4, s->stream));
+    CU(cudaMemsetAsync(s->occ, 0, 2 * (size_t)s->ncell, s->stream));
+    CU(cudaMemsetAsync(s->cellprev, 0xff, 2 * np * 4, s->stream));
     CU(cudaStreamSynchronize(s->stream));
     return SIM_OK;
 }
@@ -855,6 +936,7 @@ extern "C" int sim_write_peds(sim_t *s, const void *x, const void *y, const void
 extern "C" int sim_set_time(sim_t *s, double t, double dt)
 {
     if (!s) return SIM_EINVAL;
+    s->binned = false;
     Ctl c;
     CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
     CU(cudaStreamSynchronize(s->stream));
@@ -879,6 +961,7 @@ extern "C" int sim_set_time(sim_t *s, double t, double dt)
 extern "C" int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete)
 {
     if (!s) return SIM_EINVAL;
+    s->binned = false;
     Ctl c;
     CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
     CU(cudaStreamSynchronize(s->stream));
@@ -898,7 +981,9 @@ extern "C" void sim_destroy(sim_t *s)
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     if (s->stream2) cudaStreamDestroy(s->stream2);
     if (s->ev_fork) cudaEventDestroy(s->ev_fork);
-    if (s->ev_join) cudaEventDestroy(s->ev_join);
+    if (s->ev_ped) cudaEventDestroy(s->ev_ped);
+    if (s->ev_occ) cudaEventDestroy(s->ev_occ);
+    if (s->ev_tail) cudaEventDestroy(s->ev_tail);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
 }

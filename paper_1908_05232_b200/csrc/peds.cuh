@@ -35,13 +35,25 @@ struct PedArgs {
     int32_t *key, *off;              // per slot of A: bin key, rank inside the bin
     int32_t *count;                  // [nbins+1] (zeroed by the scan after use)
     int32_t *start;                  // [nbins+2] exclusive scan
-    int32_t *cellprev;               // per slot: cell whose occupancy this slot set last step, or -1
-    uint8_t *occ;                    // [ncell] N_p of the current step, saturated at 255
+    // N_p per cell is double-buffered by flood parity: the binning chain of step n+1 runs beside the
+    // flood step n, which is still reading the N_p of step n (buffer ctl->parity)
+    int32_t *cellprev;               // [2][n] per slot: cell whose occupancy this slot set the last time this buffer was filled, or -1
+    uint8_t *occ;                    // [2][ncell] N_p, saturated at 255
+    size_t cellprev_stride, occ_stride;
+    int pipelined;                   // 1: fill buffer ctl->occ_next (published by the pedestrian step of the step before); 0: ctl->parity
     const uint8_t *mask;             // [ncell] 1 = solid
     const uint8_t *nav;              // [n_targets][ncell]
     const T *h[2], *qx[2], *qy[2];   // flood state (level n is [ctl->parity])
     Ctl *ctl;
 };
+
+// Which N_p buffer a kernel of the binning chain fills, or -1 if the chain must not run.
+// Pipelined (beside the tail kernel of the step before, which is rewriting parity and halt):
+// the decision was taken by the pedestrian step before it; otherwise the control block is stable.
+template <typename T> __device__ __forceinline__ int chain_sel(const PedArgs<T> &a)
+{
+    return a.pipelined ? a.ctl->occ_next : (a.ctl->halt ? -1 : a.ctl->parity);
+}
 
 template <typename T> __device__ __forceinline__ int cell_of(T x, T inv, int n)
 {
@@ -56,7 +68,8 @@ template <typename T> __device__ __forceinline__ int cell_of(T x, T inv, int n)
 template <typename T>
 __global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int clear_occ)
 {
-    if (a.ctl->halt) return;
+    const int sel = chain_sel(a);
+    if (sel < 0) return;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= a.n) return;
     const unsigned lanes = __activemask();
@@ -75,8 +88,8 @@ __global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int cl
     a.off[s] = base + __popc(peers & ((1u << lane) - 1u));
     a.A.cell[s] = cell;
     if (clear_occ) {
-        const int c = a.cellprev[s];
-        if (c >= 0) a.occ[c] = 0;      // sparse clear: only cells that were set (no dense memset)
+        const int c = a.cellprev[sel * a.cellprev_stride + s];
+        if (c >= 0) a.occ[sel * a.occ_stride + c] = 0;      // sparse clear: only cells that were set (no dense memset)
     }
 }
 
@@ -89,11 +102,11 @@ __global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int cl
 constexpr int SCAN_THREADS = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 
 __global__ void __launch_bounds__(SCAN_THREADS) scan_bins_kernel(int32_t *count, int32_t *start, int n_items,
-                                                                 unsigned long long *status, Ctl *ctl)
+                                                                 unsigned long long *status, Ctl *ctl, int pipelined)
 {
     __shared__ int warp_sum[SCAN_THREADS / 32];
     __shared__ int tile_s, excl_s;
-    if (ctl->halt) return;
+    if (pipelined ? ctl->occ_next < 0 : ctl->halt != 0) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) tile_s = (int)atomicAdd(&ctl->scan_ticket, 1u);
     __syncthreads();
@@ -165,9 +178,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_bins_kernel(int32_t *count,
 template <typename T>
 __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
 {
-    if (a.ctl->halt) return;
+    if (chain_sel(a) < 0) return;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= a.n) return;
+    if (s == 0) { a.ctl->scan_ticket = 0u; a.ctl->scan_epoch += 1u; }   // the scan before me is done: re-arm it for the next chain
     const int d = a.start[a.key[s]] + a.off[s];
     const T x = a.A.x[s], y = a.A.y[s];
     a.B.x[d] = x; a.B.y[d] = y; a.bxy[d] = VecN<T, 2>{x, y};
@@ -185,17 +199,19 @@ __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
 template <typename T>
 __global__ void __launch_bounds__(256) ped_occ_kernel(PedArgs<T> a)
 {
-    if (a.ctl->halt) return;
+    const int sel = chain_sel(a);
+    if (sel < 0) return;
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
     if (d >= a.n) return;
-    if (!a.B.active[d]) { a.cellprev[d] = -1; return; }
+    int32_t *cellprev = a.cellprev + sel * a.cellprev_stride;
+    if (!a.B.active[d]) { cellprev[d] = -1; return; }
     const int c = a.B.cell[d];
     const int b = ((c / a.nx) / a.kbin) * a.nbx + (c % a.nx) / a.kbin;
     int same = 0, lower = 0;
     for (int j = a.start[b]; j < a.start[b + 1]; ++j)
         if (a.B.cell[j] == c) { same += 1; lower += (j < d); }
-    if (lower == 0) a.occ[c] = (uint8_t)min(same, 255);
-    a.cellprev[d] = c;
+    if (lower == 0) a.occ[sel * a.occ_stride + c] = (uint8_t)min(same, 255);
+    cellprev[d] = c;
 }
 
 // A_s exp((2r - d)/B_s) / d for the pair at squared distance d2 (C24)
@@ -218,8 +234,10 @@ __device__ __forceinline__ double pair_force(const PedArgs<double> &a, double d2
 template <typename T>
 __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
 {
-    if (a.ctl->halt) return;
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    // for the binning chain of the next step, which runs beside this step's tail kernel: go / no go
+    if (d == 0) a.ctl->occ_next = a.ctl->halt ? -1 : (a.ctl->parity ^ 1);
+    if (a.ctl->halt) return;
     if (d >= a.n) return;
     const PedSoA<T> &B = a.B, &A = a.A;
     const T x = B.x[d], y = B.y[d], vx = B.vx[d], vy = B.vy[d], vpref = B.vpref[d];
@@ -370,7 +388,6 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
         c->t += c->dt;
         c->step += 1;
         c->parity ^= 1;
-        c->scan_epoch += 1;
     }
     const double lam = __longlong_as_double((long long)c->lam_bits);
     double dt = c->dt_max;
@@ -378,7 +395,6 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
     if (c->t + dt > c->t_end) dt = fmax(0.0, c->t_end - c->t);
     c->dt = dt;
     c->lam_bits = 0ull;
-    c->scan_ticket = 0u;
     c->halt = (c->t >= c->t_end) ? 1 : 0;
     c->q_in = hydrograph(a.hydro_t, a.hydro_q, a.n_hydro, c->t) * a.inv_inflow_length;
 }

@@ -46,3 +46,27 @@ def mixed(a, b):
     if b.size == 0:
         return 0.0
     return float(np.max(np.abs(a - b))) / max(float(np.max(np.abs(b))), 1e-300)
+
+
+def force_magnitude_sum(x, y, sc):
+    """S_i = sum over partners within R_int of |f_ij| = A_s exp((2r - d)/B_s) (C24): the
+    scale that the rounding of the social-force sum is relative to.  Agents in a dense crowd sit
+    between forces of thousands of m/s2 that nearly cancel, so their new velocity carries an
+    absolute error of about eps * dt * S_i whatever the order of summation."""
+    from scipy.spatial import cKDTree
+    x = np.asarray(x, np.float64); y = np.asarray(y, np.float64)
+    S_i = np.zeros(x.shape[0])
+    if x.shape[0] > 1:
+        pr = cKDTree(np.c_[x, y]).query_pairs(sc.R_int, output_type="ndarray")
+        d = np.hypot(x[pr[:, 0]] - x[pr[:, 1]], y[pr[:, 0]] - y[pr[:, 1]])
+        f = sc.A_s * np.exp((2.0 * sc.radius - d) / sc.B_s)
+        np.add.at(S_i, pr[:, 0], f); np.add.at(S_i, pr[:, 1], f)
+    return S_i
+
+
+def force_sum_tolerance(x, y, sc, dt):
+    """absolute tolerance on a new velocity component from the conditioning of the force sum: each
+    term carries <= 16 ulp (ex2/rsqrt.approx and the rounding of the exponent argument d/B_s <= 12.5
+    in fp32; a few ulp in fp64), the sum is multiplied by dt."""
+    eps = 2.0 ** -23 if sc.real_bits == 32 else 2.0 ** -52
+    return 16.0 * eps * dt * force_magnitude_sum(x, y, sc)

@@ -17,6 +17,7 @@ import pytest
 
 import oracle
 from paper_1908_05232_b200 import binding, scenarios as S
+from gpu_common import force_sum_tolerance
 
 pytestmark = pytest.mark.gpu
 
@@ -48,20 +49,6 @@ def _windows(sc, rng, n_random):
         if n_random % 2 == 0 or 0.1 < frac < 0.9:
             wins.append((i0, j0)); n_random -= 1
     return wins
-
-
-def _force_magnitude_sum(sub, sc):
-    """S_i = sum over partners within R_int of |f_ij| = A_s exp((2r - d)/B_s) (C24): the
-    scale that fp32 rounding of the social-force sum is relative to."""
-    S_i = np.zeros(sub.n_peds)
-    if sub.n_peds > 1:
-        from scipy.spatial import cKDTree
-        x, y = sub.px.astype(np.float64), sub.py.astype(np.float64)
-        pr = cKDTree(np.c_[x, y]).query_pairs(sc.R_int, output_type="ndarray")
-        d = np.hypot(x[pr[:, 0]] - x[pr[:, 1]], y[pr[:, 0]] - y[pr[:, 1]])
-        f = sc.A_s * np.exp((2.0 * sc.radius - d) / sc.B_s)
-        np.add.at(S_i, pr[:, 0], f); np.add.at(S_i, pr[:, 1], f)
-    return S_i
 
 
 def _near_threshold(sub, R_int):
@@ -146,7 +133,7 @@ def test_full_size_single_step_on_sampled_windows(cfg, n_random):
             ex = np.maximum(np.abs(pa["x"][ids] - (pb["x"] + i0 * sc.dx)), np.abs(pa["y"][ids] - (pb["y"] + j0 * sc.dy))) / L
             # fp32 sum of pair forces: each term carries <= 16 ulp (ex2/rsqrt.approx and the rounding of
             # the exponent argument d/B_s <= 12.5), the sum is multiplied by dt
-            tol_v = TOL + 16.0 * 2.0 ** -23 * dt * _force_magnitude_sum(sub, sc) / vscale
+            tol_v = TOL + force_sum_tolerance(sub.px, sub.py, sc, dt) / vscale
             bad = core & ((ev > tol_v) | (ex > TOL))
             assert not np.any(bad & ~skip), (cfg, i0, j0, np.flatnonzero(bad & ~skip)[:8], float(ev[core].max()))
             assert int((bad & skip).sum()) <= max(2, c.size // 200)
