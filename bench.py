@@ -33,6 +33,9 @@ import numpy as np  # noqa: E402
 
 FLOOD_BYTES_PER_CELL = 33        # fp32: read h,qx,qy,z,n0 (20) + N_p (1) ; write h,qx,qy (12)  [DESIGN.md 6]
 PED_BYTES_PER_AGENT = 175        # key+count 17, scatter 72, step 85
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the flood kernel, from the committed
+# ncu --set full capture (profiles/r1_final_ncu_full_c5.md); only for the exact workload profiled
+NCU_TRAFFIC_BYTES = {(5, 4): 1.582797e9 + 771.306e6}
 
 
 def peaks():
@@ -133,10 +136,18 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def aggregate(ms_max, world, ncell, done, active):
+    """Whole-job numbers from the max-over-ranks time: `world` replicas each advanced `ncell` cells
+    and `active` pedestrians by `done` coupled steps in `ms_max` milliseconds."""
+    sec = ms_max * 1e-3
+    return {"value": world * ncell * done / sec, "ms_per_step": ms_max / max(done, 1),
+            "coupled_steps_per_s": world * done / sec, "agent_updates_per_s": world * active * done / sec}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_1908_05232_b200 import binding, build
+    from paper_1908_05232_b200 import binding, build, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -185,10 +196,7 @@ def run_ours(args):
     st1 = g.stats()
     done = st1["step"] - st0["step"]
     active = npeds - st0["hist"][5]
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = replicas.max_over_ranks(ms, device="cuda")
 
     # ---- per-kernel durations, CUDA events around every launch (same state, continuing)
     KP = min(K, 100)
@@ -226,10 +234,7 @@ def run_ours(args):
     ste = g.stats()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - tt0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, device="cuda")
     e2e_done = KE
 
     if rank != 0:
@@ -246,14 +251,14 @@ def run_ours(args):
     else:
         cpu = None
 
-    value = world * ncell * done / (ms_max * 1e-3)
+    agg = aggregate(ms_max, world, ncell, done, active)
     line = {
-        "metric": "flood cell-updates/s (coupled step)", "value": value, "unit": "cell-updates/s",
-        "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_max / max(done, 1),
+        "metric": "flood cell-updates/s (coupled step)", "value": agg["value"], "unit": "cell-updates/s",
+        "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": agg["ms_per_step"],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if sc.real_bits == 32 else "f64", "data": "synthetic",
-        "coupled_steps_per_s": world * done / (ms_max * 1e-3),
-        "agent_updates_per_s": world * active * done / (ms_max * 1e-3),
+        "coupled_steps_per_s": agg["coupled_steps_per_s"],
+        "agent_updates_per_s": agg["agent_updates_per_s"],
         "steps_executed": done,
         "config": {"workload": f"config{args.config}: {sc.name}", "nx": sc.nx, "ny": sc.ny, "dx": sc.dx,
                    "pedestrians": npeds, "active_pedestrians": active,
@@ -268,7 +273,10 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "kernel": ("flood_cell_kernel", "flood_tile_kernel", "flood_march_kernel", "flood_march2_kernel", "flood_tmarch_kernel")[variant] + ("<float>" if sc.real_bits == 32 else "<double>"),
                      "achieved": flood_gbs, "peak": peak, "unit": "GB/s", "frac": flood_gbs / peak,
                      "peak_source": peak_src, "frac_of_8TBs_spec": flood_gbs / 8000.0,
-                     "bytes_per_cell": fb, "kernel_ms": flood_ms, "traffic": None,
+                     "bytes_per_cell": fb, "kernel_ms": flood_ms,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.config, variant)) if args.march_rows == 0 else None,
+                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_final_ncu_full_c5.md)",
+                     "algorithmic_bytes": ncell * fb,
                      "timed_with": f"cudaEvent before each launch over {KP} steps (sim_step_profiled) right after the timed region"},
         "kernels_ms_per_step": {k: v / KP for k, v in kms.items()},
         "ped_roofline": {"bound": "hbm", "kernels": "bin_count+bin_scan+scatter+occupancy+ped_step", "achieved": ped_gbs, "peak": peak,
