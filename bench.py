@@ -120,7 +120,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    steps = min(args.steps, {1: 100, 2: 200, 3: 200, 4: 12, 5: 4}[args.config])
+    steps = min(args.steps, {1: 1000, 2: 2000, 3: 2000, 4: 24, 5: 20}[args.config])
     warm = min(args.warmup, 1)
     cps, aps, sps, desc = oracle_run(args.config, steps, warm)
     line = {
@@ -243,7 +243,7 @@ def run_ours(args):
         return
 
     # ---- CPU oracle, bounded sample (reported baseline, not the target)
-    o_steps = {1: 100, 2: 100, 3: 100, 4: 8, 5: 4}[args.config]
+    o_steps = {1: 1000, 2: 2000, 3: 2000, 4: 24, 5: 20}[args.config]     # about 10 s of one host core
     if world == 1 and not args.no_cpu_baseline:
         cps, aps, sps, desc = oracle_run(args.config, o_steps, 1)
         cpu = {"value": cps, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": desc,

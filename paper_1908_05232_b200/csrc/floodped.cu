@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -146,9 +147,19 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     s->march_gx = (g->nx + MW - 1) / MW;
     // about 15 waves of 148 SMs x 6 resident CTAs (measured on 8192^2: flat optimum R = 14..24;
     // short chunks even out the dry/wet imbalance between CTAs, halo rows cost little: not DRAM-bound)
-    s->march_R = (int)(((long long)g->ny * s->march_gx) / (15 * 148 * 6));
+    const long long slots = 148 * 6;
+    s->march_R = (int)(((long long)g->ny * s->march_gx) / (15 * slots));
     if (s->march_R > MARCH_MAX_R) s->march_R = MARCH_MAX_R;
     if (s->march_R < 16) s->march_R = 16;
+    if ((long long)s->march_gx * ((g->ny + s->march_R - 1) / s->march_R) < 4 * slots) {
+        // few waves: the last, partly filled one dominates -> fit whole waves (cost ~ waves x (R + prologue))
+        long long best = -1;
+        for (int R = 8; R <= MARCH_MAX_R; ++R) {
+            const long long ctas = (long long)s->march_gx * ((g->ny + R - 1) / R);
+            const long long cost = ((ctas + slots - 1) / slots) * (R + 3);
+            if (best < 0 || cost < best) { best = cost; s->march_R = R; }
+        }
+    }
     s->march_gy = (g->ny + s->march_R - 1) / s->march_R;
     s->n_inflow = p->n_inflow_faces; s->n_hydro = p->n_hydro; s->n_line = p->n_line; s->n_targets = p->n_targets;
     return SIM_OK;
