@@ -210,6 +210,23 @@ def run_ours(args):
     nbins = -(-sc.nx // kbin) * -(-sc.ny // kbin)
     ped_gbs = (active * PED_BYTES_PER_AGENT + nbins * 12) / (ped_ms * 1e-3) / 1e9 if npeds else 0.0
 
+    # ---- the pedestrian step is bound by the MUFU (XU) pipe in dense crowds, not by HBM: count its
+    # candidate pairs from the bin occupancy (3 x 3 bins around every agent; 2 MUFU per candidate:
+    # rsqrt, ex2 -- issued for the whole warp whenever one lane is inside the cut-off)
+    xu = None
+    if npeds:
+        b = g.bin_peds()
+        cnt = np.diff(b["start"][:b["nbx"] * b["nby"] + 1]).astype(np.int64).reshape(b["nby"], b["nbx"])
+        pad = np.pad(cnt, 1)
+        nb9 = sum(pad[dj:dj + b["nby"], di:di + b["nbx"]] for dj in range(3) for di in range(3))
+        cand = float((cnt * nb9).sum())
+        ped_step_ms = kms["ped_step"] / KP
+        xu_peak = 148 * 16 * 1.965e9 / 1e12          # 16 MUFU lanes per SM and clock (4 per SMSP), 148 SMs, 1965 MHz
+        xu = {"bound": "alu", "pipe": "xu (MUFU)", "kernel": "ped_step_kernel", "achieved": 2.0 * cand / (ped_step_ms * 1e-3) / 1e12,
+              "peak": xu_peak, "unit": "T MUFU/s", "frac": 2.0 * cand / (ped_step_ms * 1e-3) / 1e12 / xu_peak,
+              "candidate_pairs_per_step": cand, "candidates_per_agent": cand / max(active, 1), "ms": ped_step_ms,
+              "peak_source": "derived: 148 SMs x 16 MUFU/clk x 1.965 GHz (DESIGN.md 7); ncu XU pipe 70.6 % (profiles/r1_final_ncu_full_c5.md)"}
+
     # ---- end to end through the C ABI with pinned HOST buffers
     host = {k: torch.empty(ncell, dtype=torch.float32 if real is np.float32 else torch.float64).pin_memory()
             for k in ("h", "qx", "qy")}
@@ -280,7 +297,9 @@ def run_ours(args):
                      "timed_with": f"cudaEvent before each launch over {KP} steps (sim_step_profiled) right after the timed region"},
         "kernels_ms_per_step": {k: v / KP for k, v in kms.items()},
         "ped_roofline": {"bound": "hbm", "kernels": "bin_count+bin_scan+scatter+occupancy+ped_step", "achieved": ped_gbs, "peak": peak,
-                         "unit": "GB/s", "frac": ped_gbs / peak, "ms": ped_ms},
+                         "unit": "GB/s", "frac": ped_gbs / peak, "ms": ped_ms,
+                         "note": "byte view of the whole pedestrian branch; ped_step itself is XU-bound, see ped_step_roofline"},
+        "ped_step_roofline": xu,
         "cpu_baseline": cpu,
         "final": {"t": st1["t"], "volume": st1["volume"], "max_h": st1["max_h"], "hist": st1["hist"],
                   "neg_depth_clamps": st1["neg_depth_clamps"]},

@@ -77,6 +77,21 @@ __device__ __forceinline__ double pow_m73(double h) { return 1.0 / (h * h * cbrt
 __device__ __forceinline__ float  real_sqrt(float a)  { return sqrtf(a); }
 __device__ __forceinline__ double real_sqrt(double a) { return sqrt(a); }
 
+// ---- Blackwell packed single precision (FADD2 / FMUL2 / FFMA2: two IEEE fp32 operations per issue
+// slot) on pairs; min/max/select/compare and MUFU stay scalar per half
+typedef float2 f2;
+
+__device__ __forceinline__ f2 pk(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ f2 pk1(float a) { return make_float2(a, a); }
+__device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }          // folds into an operand modifier
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 max2(f2 a, f2 b) { return make_float2(fmaxf(a.x, b.x), fmaxf(a.y, b.y)); }
+__device__ __forceinline__ f2 sqrt2(f2 a) { return make_float2(fast_sqrt(a.x), fast_sqrt(a.y)); }
+__device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(fast_rcp(a.x), fast_rcp(a.y)); }
+
 __device__ __forceinline__ void atomic_max_lambda(Ctl *ctl, double lam)
 {
     // lam >= 0: the IEEE bit pattern of non-negative doubles is ordered like the integers

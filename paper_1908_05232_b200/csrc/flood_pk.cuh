@@ -16,19 +16,6 @@
 
 namespace fp {
 
-typedef float2 f2;
-
-__device__ __forceinline__ f2 pk(float a, float b) { return make_float2(a, b); }
-__device__ __forceinline__ f2 pk1(float a) { return make_float2(a, a); }
-__device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }          // folds into an operand modifier
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return __fadd2_rn(a, neg2(b)); }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
-__device__ __forceinline__ f2 max2(f2 a, f2 b) { return make_float2(fmaxf(a.x, b.x), fmaxf(a.y, b.y)); }
-__device__ __forceinline__ f2 sqrt2(f2 a) { return make_float2(fast_sqrt(a.x), fast_sqrt(a.y)); }
-__device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(fast_rcp(a.x), fast_rcp(a.y)); }
-
 // raw conserved -> (eta, u, v) of two cells (no solid cells on this path)
 __device__ __forceinline__ void prims_x2(f2 h, f2 qx, f2 qy, f2 z, float h_dry, f2 &eta, f2 &u, f2 &v)
 {

@@ -7,7 +7,6 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
-#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -601,13 +600,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     auto run = [&]() -> int {
         CU(cudaMemsetAsync(s->ws, 0, s->ws_bytes, s->stream));
         CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
-        {   // the pedestrian branch of the step graph gets the SMs first: its small kernels then hide
-            // behind the flood kernel instead of queueing after its ~15 waves of CTAs
-            int lo = 0, hi = 0;
-            CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-            const char *e = getenv("FLOODPED_PRIO");
-            CU(cudaStreamCreateWithPriority(&s->stream2, cudaStreamNonBlocking, (e && atoi(e) == 0) ? lo : hi));
-        }
+        CU(cudaStreamCreateWithFlags(&s->stream2, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
         CU(cudaEventCreateWithFlags(&s->ev_ped, cudaEventDisableTiming));
         CU(cudaEventCreateWithFlags(&s->ev_occ, cudaEventDisableTiming));
