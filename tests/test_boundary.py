@@ -51,7 +51,13 @@ def test_validation_errors_do_not_need_a_gpu(lib):
     m.grid.real_bits = 64
     m.grid.nx = 0
     assert lib.sim_workspace_bytes(C.byref(m.grid), 0, C.byref(m.params), C.byref(out)) == binding.SIM_EINVAL
-    m.grid.nx = 64
+    m.grid.nx, m.grid.ny = 65536, 65536                  # nx * ny does not fit the int32 cell index
+    assert lib.sim_workspace_bytes(C.byref(m.grid), 0, C.byref(m.params), C.byref(out)) == binding.SIM_EINVAL
+    assert b"2^31" in lib.sim_last_error(None)
+    m.grid.nx, m.grid.ny = 46340, 46340                  # the largest square that does: sizes only, no allocation
+    assert lib.sim_workspace_bytes(C.byref(m.grid), 1000, C.byref(m.params), C.byref(out)) == binding.SIM_OK
+    assert out.value > 46340 * 46340 * (6 * 8 + 2 * 8)
+    m.grid.nx, m.grid.ny = 64, 64
     m.params.R_int = 0.0
     assert lib.sim_workspace_bytes(C.byref(m.grid), 0, C.byref(m.params), C.byref(out)) == binding.SIM_EINVAL
     # NULL handle is rejected, not dereferenced
