@@ -185,32 +185,42 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     T *out_h = Ho + (size_t)y0 * nx + i, *out_qx = QXo + (size_t)y0 * nx + i, *out_qy = QYo + (size_t)y0 * nx + i;
     const int nit = R + 1;                             // iteration it handles grid row y0 + it (ring row it + 1)
 
-    if constexpr (std::is_same<T, float>::value && CPT == 2) {
-    // ---- fp32: the two columns of a thread as one packed pair (flood_pk.cuh)
-    f2 eta_q = pk(eta_p[0], eta_p[1]), u_q = pk(u_p[0], u_p[1]), v_q = pk(v_p[0], v_p[1]), z_q = pk(z_p[0], z_p[1]);
-    f2 ah2 = pk1(0.f), ax2 = pk1(0.f), ay2 = pk1(0.f), n0_q = pk1(0.f);
-    int occ_q0 = 0, occ_q1 = 0;
-    const f2 dtdx2 = pk1(dtdx), dtdy2 = pk1(dtdy), ndtdy2 = pk1(-dtdy);
+    if constexpr (std::is_same<T, float>::value && CPT % 2 == 0) {
+    // ---- fp32: the columns of a thread as NP packed pairs (flood_pk.cuh)
+    constexpr int NP = CPT / 2;
+    f2 eta_q[NP], u_q[NP], v_q[NP], z_q[NP], ah2[NP], ax2[NP], ay2[NP], n0_q[NP];
+    int occ_q[CPT];
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+        eta_q[k] = pk(eta_p[2 * k], eta_p[2 * k + 1]); u_q[k] = pk(u_p[2 * k], u_p[2 * k + 1]);
+        v_q[k] = pk(v_p[2 * k], v_p[2 * k + 1]); z_q[k] = pk(z_p[2 * k], z_p[2 * k + 1]);
+        ah2[k] = ax2[k] = ay2[k] = n0_q[k] = pk1(0.f);
+        occ_q[2 * k] = occ_q[2 * k + 1] = 0;
+    }
+    const f2 dtdx2 = pk1(dtdx), dtdy2 = pk1(dtdy), ndtdy2 = pk1(-dtdy), ndtdx2 = pk1(-dtdx);
 
     auto row = [&](auto qc, int it) {
         constexpr int b = decltype(qc)::value;
         mbar_wait(tbar, tma_par);
         const RowStage<float> &st = *reinterpret_cast<const RowStage<float> *>(sp);
-        const f2 hc = *reinterpret_cast<const f2 *>(st.h), qxc = *reinterpret_cast<const f2 *>(st.qx);
-        const f2 qyc = *reinterpret_cast<const f2 *>(st.qy), z = *reinterpret_cast<const f2 *>(st.z);
-        const f2 n0_c = *reinterpret_cast<const f2 *>(st.n0);
-        const ByteN<2> occ_c = *reinterpret_cast<const ByteN<2> *>(op);
-        f2 eta, u, v;
-        prims_x2(hc, qxc, qyc, z, h_dry, eta, u, v);
+        const VecN<f2, NP> hc = *reinterpret_cast<const VecN<f2, NP> *>(st.h), qxc = *reinterpret_cast<const VecN<f2, NP> *>(st.qx);
+        const VecN<f2, NP> qyc = *reinterpret_cast<const VecN<f2, NP> *>(st.qy), z = *reinterpret_cast<const VecN<f2, NP> *>(st.z);
+        const VecN<f2, NP> n0_c = *reinterpret_cast<const VecN<f2, NP> *>(st.n0);
+        const ByteN<CPT> occ_c = *reinterpret_cast<const ByteN<CPT> *>(op);
+        f2 eta[NP], u[NP], v[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) prims_x2(hc.v[k], qxc.v[k], qyc.v[k], z.v[k], h_dry, eta[k], u[k], v[k]);
         float *stb = my_st + b * ST_B;
-        stb[0] = eta.y; stb[NT] = u.y; stb[2 * NT] = v.y; stb[3 * NT] = z.y;
+        stb[0] = eta[NP - 1].y; stb[NT] = u[NP - 1].y; stb[2 * NT] = v[NP - 1].y; stb[3 * NT] = z.v[NP - 1].y;
 #if TM_SPLIT_BARRIER
         mbar_arrive(&xbar[b]);                         // publishes st[b] of this row and fx[b^1] of the previous one
 #endif
 
         // south faces of the current row = north faces of the previous one (normal velocity v)
-        f2 g0, g1L, g1R, g2;
-        face_eta_x2(g, eta_q, v_q, u_q, z_q, eta, v, u, z, g0, g1L, g1R, g2);
+        f2 g0[NP], g1L[NP], g1R[NP], g2[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k)
+            face_eta_x2(g, eta_q[k], v_q[k], u_q[k], z_q[k], eta[k], v[k], u[k], z.v[k], g0[k], g1L[k], g1R[k], g2[k]);
 
 #if TM_SPLIT_BARRIER
         mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
@@ -232,41 +242,71 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
             const float e0 = fe[0], e1 = fe[stride], e2 = fe[2 * stride];
             // a warp whose cells of this row hold exact zeros and receive no flux writes zeros
             // (sign bits shifted out: -0 counts as zero)
-            unsigned bits = __float_as_uint(e0) | __float_as_uint(e1) | __float_as_uint(e2)
-                          | __float_as_uint(g0.x) | __float_as_uint(g0.y) | __float_as_uint(g1L.x) | __float_as_uint(g1L.y)
-                          | __float_as_uint(g2.x) | __float_as_uint(g2.y);
+            unsigned bits = __float_as_uint(e0) | __float_as_uint(e1) | __float_as_uint(e2);
+#pragma unroll
+            for (int k = 0; k < NP; ++k)
+                bits |= __float_as_uint(g0[k].x) | __float_as_uint(g0[k].y) | __float_as_uint(g1L[k].x) | __float_as_uint(g1L[k].y)
+                      | __float_as_uint(g2[k].x) | __float_as_uint(g2[k].y);
             const bool live = live_p || (bits << 1) != 0u;
-            f2 ho = pk1(0.f), qxo = pk1(0.f), qyo = pk1(0.f);
+            VecN<f2, NP> ho, qxo, qyo;
+#pragma unroll
+            for (int k = 0; k < NP; ++k) ho.v[k] = qxo.v[k] = qyo.v[k] = pk1(0.f);
             if (__any_sync(0xffffffffu, live)) {
-                ho = fma2(ndtdy2, g0, ah2); qxo = fma2(ndtdy2, g2, ax2); qyo = fma2(ndtdy2, g1L, ay2);
-                ho.y = fmaf(-dtdx, e0, ho.y); qxo.y = fmaf(-dtdx, e1, qxo.y); qyo.y = fmaf(-dtdx, e2, qyo.y);
-                finish_hat_x2(a, dt, ho, qxo, qyo, n0_q, occ_q0, occ_q1, lam, clamp_h, clamp_n);
+#pragma unroll
+                for (int k = 0; k < NP; ++k) {
+                    ho.v[k] = fma2(ndtdy2, g0[k], ah2[k]); qxo.v[k] = fma2(ndtdy2, g2[k], ax2[k]); qyo.v[k] = fma2(ndtdy2, g1L[k], ay2[k]);
+                }
+                ho.v[NP - 1].y = fmaf(-dtdx, e0, ho.v[NP - 1].y); qxo.v[NP - 1].y = fmaf(-dtdx, e1, qxo.v[NP - 1].y);
+                qyo.v[NP - 1].y = fmaf(-dtdx, e2, qyo.v[NP - 1].y);
+#pragma unroll
+                for (int k = 0; k < NP; ++k)
+                    finish_hat_x2(a, dt, ho.v[k], qxo.v[k], qyo.v[k], n0_q[k], occ_q[2 * k], occ_q[2 * k + 1], lam, clamp_h, clamp_n);
             }
-            *reinterpret_cast<f2 *>(out_h) = ho;
-            *reinterpret_cast<f2 *>(out_qx) = qxo;
-            *reinterpret_cast<f2 *>(out_qy) = qyo;
+            *reinterpret_cast<VecN<f2, NP> *>(out_h) = ho;
+            *reinterpret_cast<VecN<f2, NP> *>(out_qx) = qxo;
+            *reinterpret_cast<VecN<f2, NP> *>(out_qy) = qyo;
             out_h += nx; out_qx += nx; out_qy += nx;
         }
         if (it < R) {                                  // enter row y0 + it: west faces, start its accumulators
             const float *sl = first_thread ? &s.sw[0][it] : stb - 1;
             const int stride = first_thread ? MARCH_MAX_R : NT;
-            // face .x: (left neighbour | my column 0), face .y: (my column 0 | my column 1)
-            f2 f0, f1L, f1R, f2v;
-            face_eta_x2(g, pk(sl[0], eta.x), pk(sl[stride], u.x), pk(sl[2 * stride], v.x), pk(sl[3 * stride], z.x),
-                        eta, u, v, z, f0, f1L, f1R, f2v);
+            // pair k: face .x = (column 2k-1 | column 2k), face .y = (column 2k | column 2k+1)
+            f2 f0[NP], f1L[NP], f1R[NP], f2v[NP];
+#pragma unroll
+            for (int k = 0; k < NP; ++k) {
+                const f2 le = k == 0 ? pk(sl[0], eta[0].x) : pk(eta[k - 1].y, eta[k].x);
+                const f2 lu = k == 0 ? pk(sl[stride], u[0].x) : pk(u[k - 1].y, u[k].x);
+                const f2 lv = k == 0 ? pk(sl[2 * stride], v[0].x) : pk(v[k - 1].y, v[k].x);
+                const f2 lz = k == 0 ? pk(sl[3 * stride], z.v[0].x) : pk(z.v[k - 1].y, z.v[k].x);
+                face_eta_x2(g, le, lu, lv, lz, eta[k], u[k], v[k], z.v[k], f0[k], f1L[k], f1R[k], f2v[k]);
+            }
             float *fxb = my_fx + b * FX_B;
-            fxb[0] = f0.x; fxb[NT] = f1L.x; fxb[2 * NT] = f2v.x;
-            ah2 = fma2(dtdx2, f0, fma2(dtdy2, g0, hc));
-            ax2 = fma2(dtdx2, f1R, fma2(dtdy2, g2, qxc));
-            ay2 = fma2(dtdx2, f2v, fma2(dtdy2, g1R, qyc));
-            // east face of column 0 = west face of column 1
-            ah2.x = fmaf(-dtdx, f0.y, ah2.x); ax2.x = fmaf(-dtdx, f1L.y, ax2.x); ay2.x = fmaf(-dtdx, f2v.y, ay2.x);
-            const unsigned ab = __float_as_uint(ah2.x) | __float_as_uint(ah2.y) | __float_as_uint(ax2.x)
-                              | __float_as_uint(ax2.y) | __float_as_uint(ay2.x) | __float_as_uint(ay2.y);
+            fxb[0] = f0[0].x; fxb[NT] = f1L[0].x; fxb[2 * NT] = f2v[0].x;
+            unsigned ab = 0u;
+#pragma unroll
+            for (int k = 0; k < NP; ++k) {
+                ah2[k] = fma2(dtdx2, f0[k], fma2(dtdy2, g0[k], hc.v[k]));
+                ax2[k] = fma2(dtdx2, f1R[k], fma2(dtdy2, g2[k], qxc.v[k]));
+                ay2[k] = fma2(dtdx2, f2v[k], fma2(dtdy2, g1R[k], qyc.v[k]));
+                if (k < NP - 1) {                      // east faces of both columns: the next west faces
+                    ah2[k] = fma2(ndtdx2, pk(f0[k].y, f0[k + 1].x), ah2[k]);
+                    ax2[k] = fma2(ndtdx2, pk(f1L[k].y, f1L[k + 1].x), ax2[k]);
+                    ay2[k] = fma2(ndtdx2, pk(f2v[k].y, f2v[k + 1].x), ay2[k]);
+                } else {                               // east face of the first column; the second one's comes from the neighbour
+                    ah2[k].x = fmaf(-dtdx, f0[k].y, ah2[k].x); ax2[k].x = fmaf(-dtdx, f1L[k].y, ax2[k].x);
+                    ay2[k].x = fmaf(-dtdx, f2v[k].y, ay2[k].x);
+                }
+                ab |= __float_as_uint(ah2[k].x) | __float_as_uint(ah2[k].y) | __float_as_uint(ax2[k].x)
+                    | __float_as_uint(ax2[k].y) | __float_as_uint(ay2[k].x) | __float_as_uint(ay2[k].y);
+            }
             live_p = (ab << 1) != 0u;
         }
-        eta_q = eta; u_q = u; v_q = v; z_q = z;
-        n0_q = n0_c; occ_q0 = a.couple ? (int)occ_c.v[0] : 0; occ_q1 = a.couple ? (int)occ_c.v[1] : 0;
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            eta_q[k] = eta[k]; u_q[k] = u[k]; v_q[k] = v[k]; z_q[k] = z.v[k];
+            n0_q[k] = n0_c.v[k];
+            occ_q[2 * k] = a.couple ? (int)occ_c.v[2 * k] : 0; occ_q[2 * k + 1] = a.couple ? (int)occ_c.v[2 * k + 1] : 0;
+        }
     };
 
     for (int base = 0; base < nit; base += 2) {
