@@ -236,7 +236,7 @@ def run_ours(args):
     p = g.read_peds()
     pin = {k: torch.from_numpy(np.ascontiguousarray(p[k])).pin_memory() for k in ("x", "y", "vx", "vy", "timer", "fsm", "active")}
     out_f = {k: torch.empty_like(host[k]).pin_memory() for k in host}
-    KE = min(K, 200)
+    KE = K
     h2d = 3 * ncell * host["h"].element_size() + sum(v.numel() * v.element_size() for v in pin.values())
     d2h = 3 * ncell * host["h"].element_size() + npeds * (5 * host["h"].element_size() + 3 + 4)
     barrier()

@@ -247,22 +247,25 @@ __global__ void __launch_bounds__(MW, sizeof(T) == 4 ? 4 : 2) flood_march_kernel
     }
 }
 
-// 1 = the chunk must take the general path: it touches the domain edge, or a solid cell lies in
-// it or in its one-cell halo.  One CTA per chunk; rerun whenever the bed array is rewritten.
+// Which path a chunk takes: 1 = it touches the domain edge (general path: bounds checks, wall
+// ghosts, inflow); 2 = interior, but a solid cell lies in it or in its one-cell halo (the row-marching
+// kernels with wall-ghost selects; variants 2 and 3 treat it like 1); 0 = interior, no solid.
+// One CTA per chunk; rerun whenever the bed array is rewritten.
 template <typename T>
 __global__ void flood_chunk_flags_kernel(const T *__restrict__ zs, int nx, int ny, int R, uint8_t *flag)
 {
     const int x0 = blockIdx.x * MW, y0 = blockIdx.y * R;
-    int bad = (x0 == 0) || (y0 == 0) || (x0 + MW >= nx) || (y0 + R >= ny);
-    if (!bad) {
+    const int edge = (x0 == 0) || (y0 == 0) || (x0 + MW >= nx) || (y0 + R >= ny);
+    int solid = 0;
+    if (!edge) {
         const int w = MW + 2, n = w * (R + 2);
         for (int k = threadIdx.x; k < n; k += blockDim.x) {
             const int i = x0 - 1 + k % w, j = y0 - 1 + k / w;
-            if (is_solid(zs[(size_t)j * nx + i])) bad = 1;
+            if (is_solid(zs[(size_t)j * nx + i])) solid = 1;
         }
     }
-    bad = __syncthreads_or(bad);
-    if (threadIdx.x == 0) flag[blockIdx.y * gridDim.x + blockIdx.x] = (uint8_t)(bad != 0);
+    solid = __syncthreads_or(solid);
+    if (threadIdx.x == 0) flag[blockIdx.y * gridDim.x + blockIdx.x] = (uint8_t)(edge ? 1 : solid ? 2 : 0);
 }
 
 }  // namespace fp

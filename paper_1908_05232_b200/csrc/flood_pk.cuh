@@ -16,18 +16,33 @@
 
 namespace fp {
 
-// raw conserved -> (eta, u, v) of two cells (no solid cells on this path)
-__device__ __forceinline__ void prims_x2(f2 h, f2 qx, f2 qy, f2 z, float h_dry, f2 &eta, f2 &u, f2 &v)
+// raw conserved -> (eta, u, v) of two cells; SOLID: a solid cell (z = +inf) holds h = q = 0, eta = +inf
+template <bool SOLID>
+__device__ __forceinline__ void prims_x2(f2 &h, f2 &qx, f2 &qy, f2 z, float h_dry, f2 &eta, f2 &u, f2 &v)
 {
+    if (SOLID) {
+        if (is_solid(z.x)) { h.x = qx.x = qy.x = 0.f; }
+        if (is_solid(z.y)) { h.y = qx.y = qy.y = 0.f; }
+    }
     const f2 r = pk(h.x > h_dry ? fast_rcp(h.x) : 0.f, h.y > h_dry ? fast_rcp(h.y) : 0.f);
     u = mul2(qx, r); v = mul2(qy, r);
     eta = add2(h, z);
 }
 
-// two faces at once; VOTE as in face_eta(): a warp none of whose faces is wet skips the flux
+// two faces at once; VOTE as in face_eta(): a warp none of whose faces is wet skips the flux.
+// SOLID: a solid side is replaced by the wall ghost of the other side (C13, C16), as in face_eta().
+template <bool SOLID>
 __device__ __forceinline__ void face_eta_x2(float g, f2 etaL, f2 uL, f2 vL, f2 zL, f2 etaR, f2 uR, f2 vR, f2 zR,
                                             f2 &f0, f2 &f1L, f2 &f1R, f2 &f2_)
 {
+    if (SOLID) {
+        const bool l0 = is_solid(zL.x), l1 = is_solid(zL.y);
+        if (l0) { etaL.x = etaR.x; uL.x = -uR.x; vL.x = vR.x; zL.x = zR.x; }
+        if (l1) { etaL.y = etaR.y; uL.y = -uR.y; vL.y = vR.y; zL.y = zR.y; }
+        const bool r0 = is_solid(zR.x), r1 = is_solid(zR.y);
+        if (r0) { etaR.x = etaL.x; uR.x = -uL.x; vR.x = vL.x; zR.x = zL.x; }
+        if (r1) { etaR.y = etaL.y; uR.y = -uL.y; vR.y = vL.y; zR.y = zL.y; }
+    }
     const f2 zf = max2(zL, zR);
     const f2 hL = max2(pk1(0.f), sub2(etaL, zf));
     const f2 hR = max2(pk1(0.f), sub2(etaR, zf));

@@ -95,7 +95,7 @@ __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, 
 //   __syncthreads.  The ring slot is refilled after that wait (all threads have their values in
 //   registers before they arrive).  The TMA issue sits in a warp-uniform branch with one elected
 //   lane, its addresses derived from uniform values only.
-template <typename T, int CPT, int STAGES>
+template <typename T, int CPT, int STAGES, bool SOLID>
 __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, CPT> &s, RowStage<T> *ring,
                                           uint64_t *bars, int x0, int y0, int R)
 {
@@ -134,10 +134,10 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         Raw4<T> r = march_load<T, false>(H, QX, QY, Z, x0 + MW, j, nx, a.ny);
         Raw4<T> w = march_load<T, false>(H, QX, QY, Z, x0 - 1, j, nx, a.ny);
         T el, ul, vl, er_, ur, vr, ew, uw, vw, f0, f1L, f1R, f2;
-        march_prims<T, false>(l, h_dry, el, ul, vl);
-        march_prims<T, false>(r, h_dry, er_, ur, vr);
-        march_prims<T, false>(w, h_dry, ew, uw, vw);
-        face_eta<T, false, false>(g, el, ul, vl, l.z, er_, ur, vr, r.z, f0, f1L, f1R, f2);
+        march_prims<T, SOLID>(l, h_dry, el, ul, vl);
+        march_prims<T, SOLID>(r, h_dry, er_, ur, vr);
+        march_prims<T, SOLID>(w, h_dry, ew, uw, vw);
+        face_eta<T, SOLID, false>(g, el, ul, vl, l.z, er_, ur, vr, r.z, f0, f1L, f1R, f2);
         s.er[0][k] = f0; s.er[1][k] = f1L; s.er[2][k] = f2;
         s.sw[0][k] = ew; s.sw[1][k] = uw; s.sw[2][k] = vw; s.sw[3][k] = w.z;
     }
@@ -154,7 +154,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
 #pragma unroll
         for (int k = 0; k < CPT; ++k) {
             Raw4<T> q{h.v[k], qx.v[k], qy.v[k], z.v[k]};
-            march_prims<T, false>(q, h_dry, eta_p[k], u_p[k], v_p[k]);
+            march_prims<T, SOLID>(q, h_dry, eta_p[k], u_p[k], v_p[k]);
             z_p[k] = q.z;
         }
     }
@@ -203,13 +203,14 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         constexpr int b = decltype(qc)::value;
         mbar_wait(tbar, tma_par);
         const RowStage<float> &st = *reinterpret_cast<const RowStage<float> *>(sp);
-        const VecN<f2, NP> hc = *reinterpret_cast<const VecN<f2, NP> *>(st.h), qxc = *reinterpret_cast<const VecN<f2, NP> *>(st.qx);
-        const VecN<f2, NP> qyc = *reinterpret_cast<const VecN<f2, NP> *>(st.qy), z = *reinterpret_cast<const VecN<f2, NP> *>(st.z);
+        VecN<f2, NP> hc = *reinterpret_cast<const VecN<f2, NP> *>(st.h), qxc = *reinterpret_cast<const VecN<f2, NP> *>(st.qx);
+        VecN<f2, NP> qyc = *reinterpret_cast<const VecN<f2, NP> *>(st.qy);
+        const VecN<f2, NP> z = *reinterpret_cast<const VecN<f2, NP> *>(st.z);
         const VecN<f2, NP> n0_c = *reinterpret_cast<const VecN<f2, NP> *>(st.n0);
         const ByteN<CPT> occ_c = *reinterpret_cast<const ByteN<CPT> *>(op);
         f2 eta[NP], u[NP], v[NP];
 #pragma unroll
-        for (int k = 0; k < NP; ++k) prims_x2(hc.v[k], qxc.v[k], qyc.v[k], z.v[k], h_dry, eta[k], u[k], v[k]);
+        for (int k = 0; k < NP; ++k) prims_x2<SOLID>(hc.v[k], qxc.v[k], qyc.v[k], z.v[k], h_dry, eta[k], u[k], v[k]);
         float *stb = my_st + b * ST_B;
         stb[0] = eta[NP - 1].y; stb[NT] = u[NP - 1].y; stb[2 * NT] = v[NP - 1].y; stb[3 * NT] = z.v[NP - 1].y;
 #if TM_SPLIT_BARRIER
@@ -220,7 +221,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         f2 g0[NP], g1L[NP], g1R[NP], g2[NP];
 #pragma unroll
         for (int k = 0; k < NP; ++k)
-            face_eta_x2(g, eta_q[k], v_q[k], u_q[k], z_q[k], eta[k], v[k], u[k], z.v[k], g0[k], g1L[k], g1R[k], g2[k]);
+            face_eta_x2<SOLID>(g, eta_q[k], v_q[k], u_q[k], z_q[k], eta[k], v[k], u[k], z.v[k], g0[k], g1L[k], g1R[k], g2[k]);
 
 #if TM_SPLIT_BARRIER
         mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
@@ -258,6 +259,13 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 }
                 ho.v[NP - 1].y = fmaf(-dtdx, e0, ho.v[NP - 1].y); qxo.v[NP - 1].y = fmaf(-dtdx, e1, qxo.v[NP - 1].y);
                 qyo.v[NP - 1].y = fmaf(-dtdx, e2, qyo.v[NP - 1].y);
+                if (SOLID) {                           // nothing moves in a solid cell (and no clamp is counted)
+#pragma unroll
+                    for (int k = 0; k < NP; ++k) {
+                        if (is_solid(z_q[k].x)) { ho.v[k].x = qxo.v[k].x = qyo.v[k].x = 0.f; }
+                        if (is_solid(z_q[k].y)) { ho.v[k].y = qxo.v[k].y = qyo.v[k].y = 0.f; }
+                    }
+                }
 #pragma unroll
                 for (int k = 0; k < NP; ++k)
                     finish_hat_x2(a, dt, ho.v[k], qxo.v[k], qyo.v[k], n0_q[k], occ_q[2 * k], occ_q[2 * k + 1], lam, clamp_h, clamp_n);
@@ -278,7 +286,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 const f2 lu = k == 0 ? pk(sl[stride], u[0].x) : pk(u[k - 1].y, u[k].x);
                 const f2 lv = k == 0 ? pk(sl[2 * stride], v[0].x) : pk(v[k - 1].y, v[k].x);
                 const f2 lz = k == 0 ? pk(sl[3 * stride], z.v[0].x) : pk(z.v[k - 1].y, z.v[k].x);
-                face_eta_x2(g, le, lu, lv, lz, eta[k], u[k], v[k], z.v[k], f0[k], f1L[k], f1R[k], f2v[k]);
+                face_eta_x2<SOLID>(g, le, lu, lv, lz, eta[k], u[k], v[k], z.v[k], f0[k], f1L[k], f1R[k], f2v[k]);
             }
             float *fxb = my_fx + b * FX_B;
             fxb[0] = f0[0].x; fxb[NT] = f1L[0].x; fxb[2 * NT] = f2v[0].x;
@@ -329,7 +337,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
 #pragma unroll
         for (int k = 0; k < CPT; ++k) {
             Raw4<T> qq{hv.v[k], qxv.v[k], qyv.v[k], zv.v[k]};
-            march_prims<T, false>(qq, h_dry, eta[k], u[k], v[k]);
+            march_prims<T, SOLID>(qq, h_dry, eta[k], u[k], v[k]);
             z[k] = qq.z; hc[k] = qq.h; qxc[k] = qq.qx; qyc[k] = qq.qy;
         }
         T *stb = my_st + b * ST_B;
@@ -342,7 +350,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         T g0[CPT], g1L[CPT], g1R[CPT], g2[CPT];
 #pragma unroll
         for (int k = 0; k < CPT; ++k)
-            face_eta<T, false, true>(g, eta_p[k], v_p[k], u_p[k], z_p[k], eta[k], v[k], u[k], z[k], g0[k], g1L[k], g1R[k], g2[k]);
+            face_eta<T, SOLID, true>(g, eta_p[k], v_p[k], u_p[k], z_p[k], eta[k], v[k], u[k], z[k], g0[k], g1L[k], g1R[k], g2[k]);
 
 #if TM_SPLIT_BARRIER
         mbar_wait(&xbar[b], xpar);                     // use it/2 of xbar[b]
@@ -374,6 +382,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 for (int k = 0; k < CPT; ++k) {
                     T hn = ah[k] - dtdy * g0[k], qxn = ax[k] - dtdy * g2[k], qyn = ay[k] - dtdy * g1L[k];
                     if (k == CPT - 1) { hn -= dtdx * e0; qxn -= dtdx * e1; qyn -= dtdx * e2; }
+                    if (SOLID && is_solid(z_p[k])) { hn = qxn = qyn = T(0); }
                     finish_hat2(a, dt, hn, qxn, qyn, n0_p[k], occ_p[k], lam, clamp_h, clamp_n);
                     ho.v[k] = hn; qxo.v[k] = qxn; qyo.v[k] = qyn;
                 }
@@ -387,11 +396,11 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
             const T *sl = first_thread ? &s.sw[0][it] : stb - 1;
             const int stride = first_thread ? MARCH_MAX_R : NT;
             T f0[CPT], f1L[CPT], f1R[CPT], f2[CPT];
-            face_eta<T, false, true>(g, sl[0], sl[stride], sl[2 * stride], sl[3 * stride], eta[0], u[0], v[0], z[0],
+            face_eta<T, SOLID, true>(g, sl[0], sl[stride], sl[2 * stride], sl[3 * stride], eta[0], u[0], v[0], z[0],
                                      f0[0], f1L[0], f1R[0], f2[0]);
 #pragma unroll
             for (int k = 1; k < CPT; ++k)
-                face_eta<T, false, true>(g, eta[k - 1], u[k - 1], v[k - 1], z[k - 1], eta[k], u[k], v[k], z[k],
+                face_eta<T, SOLID, true>(g, eta[k - 1], u[k - 1], v[k - 1], z[k - 1], eta[k], u[k], v[k], z[k],
                                          f0[k], f1L[k], f1R[k], f2[k]);
             T *fxb = my_fx + b * FX_B;
             fxb[0] = f0[0]; fxb[NT] = f1L[0]; fxb[2 * NT] = f2[0];
@@ -437,9 +446,10 @@ __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tma
     RowStage<T> *ring = reinterpret_cast<RowStage<T> *>(tm_dyn);
     uint64_t *bars = reinterpret_cast<uint64_t *>(tm_dyn + sizeof(RowStage<T>) * STAGES);
     const int x0 = blockIdx.x * MW, y0 = blockIdx.y * a.R;
-    const bool gen = a.chunk_flag[blockIdx.y * gridDim.x + blockIdx.x] != 0;
-    T lam = gen ? march2_chunk<T, CPT, true>(a, s, x0, y0, a.R)
-                : tmarch_chunk<T, CPT, STAGES>(a, s, ring, bars, x0, y0, a.R);
+    const int path = a.chunk_flag[blockIdx.y * gridDim.x + blockIdx.x];
+    T lam = path == 1 ? march2_chunk<T, CPT, true>(a, s, x0, y0, a.R)
+          : path == 2 ? tmarch_chunk<T, CPT, STAGES, true>(a, s, ring, bars, x0, y0, a.R)
+                      : tmarch_chunk<T, CPT, STAGES, false>(a, s, ring, bars, x0, y0, a.R);
     const int tid = threadIdx.x;
     for (int o = 16; o > 0; o >>= 1) lam = fmax(lam, __shfl_xor_sync(0xffffffffu, lam, o));
     __syncthreads();
