@@ -130,3 +130,78 @@ def test_step_graph_with_and_without_the_parallel_branch_gives_the_same_bits():
             assert np.array_equal(p[k], outs[0][1][k]), k
         assert np.array_equal(occ, outs[0][2])
         assert st["t"] == outs[0][3]["t"] and st["step"] == 100
+
+
+def _sparse_scenario(n=128):
+    """a flooding hall with a sparse crowd (no agent ever has two partners within R_int, so the
+    pedestrian sums have one order only and every run is bit-reproducible)"""
+    gx, gy = np.meshgrid(np.arange(8, 120, 7.0), np.arange(8, 120, 7.0))
+    sc = S.make(2, n=n, n_evac=10)
+    sc.hydro_q = sc.hydro_q * 30.0
+    walk = sc.mask.reshape(n, n) == 0
+    keep = walk[(gy.ravel() / sc.dy).astype(int), (gx.ravel() / sc.dx).astype(int)]
+    x, y = gx.ravel()[keep] * 0.5 + 0.1, gy.ravel()[keep] * 0.5 + 0.1
+    m = x.size
+    sc.px, sc.py = x.astype(np.float32), y.astype(np.float32)
+    sc.pvx = np.zeros(m, np.float32); sc.pvy = np.zeros(m, np.float32)
+    sc.pvpref = np.full(m, 0.2, np.float32); sc.prole = np.zeros(m, np.uint8)
+    return sc
+
+
+def _state(g):
+    c, p = g.read_conserved(), g.read_peds()
+    return [c["h"], c["qx"], c["qy"], p["x"], p["y"], p["vx"], p["vy"], p["state"], p["active"], g.read_occupancy()]
+
+
+def _same(a, b):
+    return all(np.array_equal(u, v) for u, v in zip(a, b))
+
+
+def test_step_counts_split_any_way_give_the_same_bits():
+    """37 steps as one call (a 32-step graph + 5 single ones), as 32 + 5, as 37 x 1, and with
+    read-backs in between (which must not disturb the prepared binning of the next step)"""
+    sc = _sparse_scenario()
+    ref = binding.Sim(sc); ref.step(37); want = _state(ref); t = ref.stats()["t"]
+    g = binding.Sim(sc); g.step(32); g.step(5)
+    assert _same(_state(g), want) and g.stats()["t"] == t
+    g = binding.Sim(sc)
+    for k in range(37):
+        g.step(1)
+        if k % 9 == 0:
+            g.read_peds(); g.stats(); g.read_flood(("h", "hr")); g.bin_peds()
+    assert _same(_state(g), want) and g.stats()["t"] == t
+
+
+def test_two_handles_on_one_gpu_do_not_disturb_each_other():
+    """replicas: two sim_t on one device, stepped alternately, equal their solo runs"""
+    sa, sb = _sparse_scenario(), S.make(1)
+    solo_a = binding.Sim(sa); solo_a.step(40); wa = _state(solo_a)
+    solo_b = binding.Sim(sb); solo_b.step(40); wb = _state(solo_b)
+    ga, gb = binding.Sim(sa), binding.Sim(sb)
+    for _ in range(8):
+        ga.step(5); gb.step(5)
+    assert _same(_state(ga), wa)
+    # Config 1 is a dense-ish crowd: compare the flood bitwise, the pedestrians within tolerance
+    got = _state(gb)
+    assert all(np.array_equal(u, v) for u, v in zip(got[:3], wb[:3])) or mixed(got[0], wb[0]) <= 1e-12
+    assert mixed(got[3], wb[3]) <= 1e-9
+
+
+def test_rows_per_chunk_do_not_change_the_flood():
+    """the chunk height of the row-marching kernel is a tuning parameter.  It moves the border
+    between chunks on the packed/TMA path and chunks on the general path (different FMA contraction),
+    so the results agree to rounding, not to the bit"""
+    rng = np.random.default_rng(5)
+    nx, ny = 1024, 160
+    jj, ii = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    z = 0.3 * (1 + np.sin(ii / 37.0) * np.cos(jj / 11.0))
+    mask = np.zeros((ny, nx), np.uint8); mask[60:70, 300:330] = 1; mask[100, 511:514] = 1
+    sc = box(nx, ny, dx=0.25, real_bits=32, z=z, h0=np.maximum(0.0, 0.35 - z), u0=rng.normal(0, 0.3, (ny, nx)),
+             v0=rng.normal(0, 0.3, (ny, nx)), mask=mask, manning=0.02, dt_max=0.02)
+    outs = []
+    for rows in (8, 19, 64):
+        g = binding.Sim(sc); g.set_flood_variant(4); g.set_march_rows(rows); g.step(6)
+        outs.append(g.read_conserved()); g.close()
+    for o in outs[1:]:
+        for k in ("h", "qx", "qy"):
+            assert mixed(o[k], outs[0][k]) <= 6 * 2e-6, (k, mixed(o[k], outs[0][k]))
