@@ -1,19 +1,26 @@
 // flood_tmarch.cuh -- variant 4 of step (F)+(T): the row-marching flood-cell update of
-// flood_march2.cuh (Eq. (2); same face_eta(), finish_hat2(), same strip/chunk geometry and
-// shared-memory exchange) with the rows of an interior chunk brought in by the TMA engine.
+// flood_march2.cuh (Eq. (2); same face flux, finish, strip/chunk geometry and shared-memory
+// exchange) with the rows of an interior chunk brought in by the TMA engine and, in fp32, the
+// arithmetic on packed pairs (flood_pk.cuh).  The default kernel from 2^22 cells.
 //
-//   Why: ncu of variant 3 (two columns per thread, 117 registers, 16 warps/SM) shows the fewest
-//   instructions per cell of all variants (195) but IPC 0.52 with long-scoreboard (global-load
-//   latency) as the dominant stall: register prefetch two rows ahead does not keep enough bytes in
-//   flight at that occupancy.  Here one elected thread issues, per row, six 1-D bulk copies
-//   (cp.async.bulk global -> shared: h, qx, qy, z, n0 of the strip's 256 columns and their N_p
-//   bytes) into a ring of STAGES row buffers, each completing on an mbarrier; the ring runs STAGES
-//   rows ahead of the arithmetic at no register cost.  The slot read in iteration r is refilled
-//   with row r+STAGES right after that iteration's __syncthreads (every thread has its values in
+//   Why TMA: ncu of variant 3 (two columns per thread, 117 registers, 16 warps/SM) showed the fewest
+//   instructions per cell of the register-prefetch variants (195) but IPC 0.52 with long-scoreboard
+//   (global-load latency) as the dominant stall: prefetching two rows ahead into registers does not
+//   keep enough bytes in flight at that occupancy.  Here one elected lane of warp 0 issues, per row,
+//   six 1-D bulk copies (cp.async.bulk global -> shared: h, qx, qy, z, n0 of the strip's 256 columns
+//   and their N_p bytes) into a ring of STAGES row buffers, each completing on an mbarrier; the ring
+//   runs STAGES rows ahead of the arithmetic at no register cost.  The slot read in iteration r is
+//   refilled with row r+STAGES right after that iteration's barrier (every thread has its values in
 //   registers by then).
 //
-//   Chunks that touch the domain edge or a solid cell (chunk_flag = 1) take march2_chunk<GEN=true>
-//   with plain loads.  Needs nx % 16 == 0 (16-byte alignment of every row segment).
+//   chunk_flag picks the path of a chunk: 0 = interior without solid cells (no selects), 2 = interior
+//   with solid cells in it or its halo (same path with wall-ghost selects, SOLID = true), 1 = touching
+//   the domain edge (march2_chunk<GEN=true>: plain loads, bounds checks, inflow).
+//   Needs nx % 16 == 0 (16-byte alignment of every row segment).
+//
+//   TM_SPLIT_BARRIER=1 builds the measured-and-dropped alternative to the per-row __syncthreads: a
+//   split-phase mbarrier (arrive after publishing, wait after the south faces), whose try_wait loop
+//   spins through more issue slots than the barrier stall it removes.
 #pragma once
 
 #include <type_traits>
@@ -86,14 +93,12 @@ __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, 
     bulk_g2s(st.occ, OCC + c, MW, bar);
 }
 
-// interior chunk (no domain edge, no solid cell in it or in its halo): rows y0-1 .. y0+R all exist
+// interior chunk (no domain edge; SOLID: solid cells in it or in its halo): rows y0-1 .. y0+R all exist
 //
 //   Synchronisation per row: the neighbour exchange (last-column state st[b], west-face flux
-//   fx[b]) goes through a SPLIT-PHASE barrier -- every thread arrives on xbar[b] right after
-//   publishing its state and waits only after the south faces, which need nothing from the
-//   neighbours, so the warp that also feeds the TMA ring no longer holds the others at a
-//   __syncthreads.  The ring slot is refilled after that wait (all threads have their values in
-//   registers before they arrive).  The TMA issue sits in a warp-uniform branch with one elected
+//   fx[b]) needs one CTA-wide barrier per row.  It sits AFTER the south faces, which need nothing
+//   from the neighbours, so the skew between warps is spent on useful work first.  The ring slot is
+//   refilled after that barrier (all threads have their values in registers by then).  The TMA issue sits in a warp-uniform branch with one elected
 //   lane, its addresses derived from uniform values only.
 template <typename T, int CPT, int STAGES, bool SOLID>
 __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, CPT> &s, RowStage<T> *ring,
@@ -112,7 +117,6 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     const T dtdx = dt * a.inv_dx, dtdy = dt * a.inv_dy;
     const T g = a.g, h_dry = a.h_dry;
     const int i = x0 + tid * CPT;
-    const int y1 = y0 + R;
     const int nrows = R + 2;                           // ring row r holds grid row y0 - 1 + r
     uint64_t *xbar = bars + STAGES;                    // exchange barriers, by row parity
 
