@@ -92,6 +92,15 @@ __device__ __forceinline__ f2 max2(f2 a, f2 b) { return make_float2(fmaxf(a.x, b
 __device__ __forceinline__ f2 sqrt2(f2 a) { return make_float2(fast_sqrt(a.x), fast_sqrt(a.y)); }
 __device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(fast_rcp(a.x), fast_rcp(a.y)); }
 
+// Programmatic dependent launch: a kernel launched with the programmatic-serialization attribute
+// may start while the kernel before it in the stream is still draining; everything it reads from
+// that kernel must come after this wait (a no-op for ordinary launches).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Let the next kernel of the stream be scheduled now: its CTAs then sit at their pdl_wait() until
+// this grid has completed and flushed, instead of being launched after it (saves the launch gap).
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_enter() { pdl_trigger(); pdl_wait(); }
+
 __device__ __forceinline__ void atomic_max_lambda(Ctl *ctl, double lam)
 {
     // lam >= 0: the IEEE bit pattern of non-negative doubles is ordered like the integers

@@ -141,6 +141,7 @@ __device__ __forceinline__ void block_max_lambda(Ctl *ctl, T lam, T *warp_scratc
 template <typename T>
 __global__ void __launch_bounds__(256) flood_cell_kernel(FloodArgs<T> a)
 {
+    pdl_enter();
     __shared__ T red[32];
     if (a.ctl->halt) return;
     const int p = a.ctl->parity;
@@ -211,6 +212,7 @@ struct TileSmem {
 template <typename T>
 __global__ void __launch_bounds__(FLOOD_TILE_THREADS, sizeof(T) == 4 ? 3 : 1) flood_tile_kernel(FloodArgs<T> a)
 {
+    pdl_enter();
     extern __shared__ __align__(32) unsigned char smem_raw[];
     TileSmem<T> &s = *reinterpret_cast<TileSmem<T> *>(smem_raw);
     if (a.ctl->halt) return;

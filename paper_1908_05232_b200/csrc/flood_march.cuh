@@ -230,6 +230,7 @@ __device__ __forceinline__ T march_chunk(const FloodArgs<T> &a, MarchSmem<T> &s,
 template <typename T>
 __global__ void __launch_bounds__(MW, sizeof(T) == 4 ? 4 : 2) flood_march_kernel(FloodArgs<T> a)
 {
+    pdl_enter();
     __shared__ MarchSmem<T> s;
     if (a.ctl->halt) return;
     const int x0 = blockIdx.x * MW, y0 = blockIdx.y * a.R;

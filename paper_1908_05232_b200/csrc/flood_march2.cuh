@@ -224,6 +224,7 @@ __device__ __forceinline__ T march2_chunk(const FloodArgs<T> &a, March2Smem<T, C
 template <typename T, int CPT>
 __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? 4 : 2) flood_march2_kernel(FloodArgs<T> a)
 {
+    pdl_enter();
     constexpr int NT = MW / CPT;
     __shared__ March2Smem<T, CPT> s;
     if (a.ctl->halt) return;

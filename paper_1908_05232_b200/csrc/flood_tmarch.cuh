@@ -443,6 +443,7 @@ template <typename T, int STAGES> constexpr size_t tmarch_dyn_smem() { return si
 template <typename T, int CPT, int STAGES, int MINB>
 __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tmarch_kernel(FloodArgs<T> a)
 {
+    pdl_enter();
     constexpr int NT = MW / CPT;
     __shared__ March2Smem<T, CPT> s;
     extern __shared__ __align__(16) unsigned char tm_dyn[];

@@ -68,6 +68,7 @@ struct sim {
     cudaStream_t stream2 = nullptr;   // second branch of the step graph (pedestrian step beside the flood step)
     cudaEvent_t ev_fork = nullptr, ev_ped = nullptr, ev_occ = nullptr, ev_tail = nullptr;
     int overlap = 1;
+    int pdl = 1;                     // programmatic dependent launch inside the step graph
     bool binned = false;             // the binning chain of the upcoming step has run on the current state
     std::string err;
 };
@@ -164,13 +165,26 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     return SIM_OK;
 }
 
+// launch with the programmatic-serialization attribute (graph mode only; see pdl_wait())
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, Args... args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <typename T, int CPT, int STAGES, int MINB>
-void launch_tmarch(const FloodArgs<T> &fa, dim3 grid, cudaStream_t st)
+void launch_tmarch(const FloodArgs<T> &fa, dim3 grid, cudaStream_t st, bool pdl)
 {
     constexpr size_t dyn = tmarch_dyn_smem<T, STAGES>();
     static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, CPT, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
     (void)once;
-    flood_tmarch_kernel<T, CPT, STAGES, MINB><<<grid, MW / CPT, dyn, st>>>(fa);
+    launch_pdl(flood_tmarch_kernel<T, CPT, STAGES, MINB>, grid, dim3(MW / CPT), dyn, st, pdl, fa);
 }
 
 template <typename T> FloodArgs<T> flood_args(const sim *s)
@@ -246,6 +260,7 @@ template <typename T> PedArgs<T> ped_args_full(const sim *s, int pipelined)
     for (int e = 0; e < s->prm.n_exit_cells; ++e) { pa.exit_i[e] = s->exit_i[e]; pa.exit_j[e] = s->exit_j[e]; }
     pa.n_exit = s->prm.n_exit_cells;
     pa.pipelined = pipelined;
+    pa.pdl_early = s->np >= 65536;   // measured: pre-scheduling the chain pays on Config 5 (-1.5 %), costs on Configs 1-3 (+8 %)
     return pa;
 }
 
@@ -261,33 +276,35 @@ template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelin
 {
     PedArgs<T> pa = ped_args_full<T>(s, pipelined);
     const int nb = (s->np + 255) / 256, n_items = s->nbins + 1;
+    const bool pdl = s->pdl && !mark.ev;              // graph mode: each kernel may start under the tail of the one before
     mark();
-    ped_bin_count_kernel<T><<<nb, 256, 0, st>>>(pa, 1);
+    CU(launch_pdl(ped_bin_count_kernel<T>, dim3(nb), dim3(256), 0, st, pdl && pipelined, pa, 1));
     mark();
-    scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, st>>>(s->count, s->start, n_items, s->scan_status, s->ctl, pipelined);
+    CU(launch_pdl(scan_bins_kernel, dim3((n_items + SCAN_TILE - 1) / SCAN_TILE), dim3(SCAN_THREADS), 0, st, pdl,
+                  s->count, s->start, n_items, s->scan_status, s->ctl, pipelined, pa.pdl_early));
     mark();
-    ped_scatter_kernel<T><<<nb, 256, 0, st>>>(pa);
+    CU(launch_pdl(ped_scatter_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
     mark();
-    ped_occ_kernel<T><<<nb, 256, 0, st>>>(pa);
+    CU(launch_pdl(ped_occ_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
     CU(cudaGetLastError());
     return SIM_OK;
 }
 
-template <typename T> void launch_flood(sim *s, cudaStream_t st)
+template <typename T> void launch_flood(sim *s, cudaStream_t st, bool pdl)
 {
     FloodArgs<T> fa = flood_args<T>(s);
     if (s->flood_variant == 4) {
-        launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st);
+        launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st, pdl);
     } else if (s->flood_variant == 3) {
-        flood_march2_kernel<T, 2><<<dim3(s->march_gx, s->march_gy), MW / 2, 0, st>>>(fa);
+        launch_pdl(flood_march2_kernel<T, 2>, dim3(s->march_gx, s->march_gy), dim3(MW / 2), 0, st, pdl, fa);
     } else if (s->flood_variant == 2) {
-        flood_march_kernel<T><<<dim3(s->march_gx, s->march_gy), MW, 0, st>>>(fa);
+        launch_pdl(flood_march_kernel<T>, dim3(s->march_gx, s->march_gy), dim3(MW), 0, st, pdl, fa);
     } else if (s->flood_variant == 1) {
         dim3 grid((s->grid.nx + TX - 1) / TX, (s->grid.ny + TY - 1) / TY);
-        flood_tile_kernel<T><<<grid, FLOOD_TILE_THREADS, sizeof(TileSmem<T>), st>>>(fa);
+        launch_pdl(flood_tile_kernel<T>, grid, dim3(FLOOD_TILE_THREADS), sizeof(TileSmem<T>), st, pdl, fa);
     } else {
         dim3 blk(32, 8), grid((s->grid.nx + 31) / 32, (s->grid.ny + 7) / 8);
-        flood_cell_kernel<T><<<grid, blk, 0, st>>>(fa);
+        launch_pdl(flood_cell_kernel<T>, grid, blk, 0, st, pdl, fa);
     }
 }
 
@@ -309,14 +326,14 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cuda
             else CU(cudaStreamWaitEvent(sp, s->ev_tail, 0));
         }
         mark();
-        ped_step_kernel<T><<<(s->np + 127) / 128, 128, 0, sp>>>(ped_args_full<T>(s, 0));
+        CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + 127) / 128), dim3(128), 0, sp, s->pdl && !ev, ped_args_full<T>(s, 0)));
         if (fork) {
             CU(cudaEventRecord(s->ev_ped, sp));
             if (!first) CU(cudaStreamWaitEvent(st, s->ev_occ, 0));     // N_p of this step, filled beside the step before
         }
     } else mark.k = 1;
     mark();
-    launch_flood<T>(s, st);
+    launch_flood<T>(s, st, s->pdl && !ev);
     if (fork) {
         int rc = enqueue_bin_chain<T>(s, sp, 1, mark);
         if (rc != SIM_OK) return rc;
@@ -324,7 +341,7 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cuda
         CU(cudaStreamWaitEvent(st, s->ev_ped, 0));
     }
     mark();
-    tail_kernel<T><<<1, 32, 0, st>>>(tail_args<T>(s), 0);
+    CU(launch_pdl(tail_kernel<T>, dim3(1), dim3(32), 0, st, s->pdl && !ev, tail_args<T>(s), 0));
     if (fork) CU(cudaEventRecord(s->ev_tail, st));
     if (peds && !fork) {
         int rc = enqueue_bin_chain<T>(s, st, 0, mark);               // after the tail: ctl->parity is that of step n+1
@@ -785,7 +802,7 @@ template <typename T> int bin_peds_t(sim *s, int32_t *key, int32_t *order, int32
         const int halt = c.halt;
         if (halt) { c.halt = 0; CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream)); }
         ped_bin_count_kernel<T><<<nb, 256, 0, s->stream>>>(pa, 0);
-        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl, 0);
+        scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl, 0, 0);
         ped_scatter_kernel<T><<<nb, 256, 0, s->stream>>>(pa);
         ped_key_by_id_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 0), s->key, np, s->ped_out_i32[0]);
         ped_gather_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 1), np, s->grid.nx, (T)1, (T)1, s->grid.ny,

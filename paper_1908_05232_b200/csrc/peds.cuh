@@ -40,6 +40,7 @@ struct PedArgs {
     int32_t *cellprev;               // [2][n] per slot: cell whose occupancy this slot set the last time this buffer was filled, or -1
     uint8_t *occ;                    // [2][ncell] N_p, saturated at 255
     size_t cellprev_stride, occ_stride;
+    int pdl_early;                   // 1: let the next kernel of the chain be scheduled at once (large crowds), see pdl_trigger()
     int pipelined;                   // 1: fill buffer ctl->occ_next (published by the pedestrian step of the step before); 0: ctl->parity
     const uint8_t *mask;             // [ncell] 1 = solid
     const uint8_t *nav;              // [n_targets][ncell]
@@ -68,6 +69,8 @@ template <typename T> __device__ __forceinline__ int cell_of(T x, T inv, int n)
 template <typename T>
 __global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int clear_occ)
 {
+    if (a.pdl_early) pdl_trigger();
+    pdl_wait();
     const int sel = chain_sel(a);
     if (sel < 0) return;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -102,10 +105,12 @@ __global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int cl
 constexpr int SCAN_THREADS = 512, SCAN_ITEMS = 16, SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;   // 8192 counts per tile: 128-bit accesses, short look-back chain
 
 __global__ void __launch_bounds__(SCAN_THREADS) scan_bins_kernel(int32_t *count, int32_t *start, int n_items,
-                                                                 unsigned long long *status, Ctl *ctl, int pipelined)
+                                                                 unsigned long long *status, Ctl *ctl, int pipelined, int pdl_early)
 {
     __shared__ int warp_sum[SCAN_THREADS / 32];
     __shared__ int tile_s, excl_s;
+    if (pdl_early) pdl_trigger();
+    pdl_wait();
     if (pipelined ? ctl->occ_next < 0 : ctl->halt != 0) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) tile_s = (int)atomicAdd(&ctl->scan_ticket, 1u);
@@ -205,6 +210,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_bins_kernel(int32_t *count,
 template <typename T>
 __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
 {
+    if (a.pdl_early) pdl_trigger();
+    pdl_wait();
     if (chain_sel(a) < 0) return;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= a.n) return;
@@ -226,6 +233,8 @@ __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
 template <typename T>
 __global__ void __launch_bounds__(256) ped_occ_kernel(PedArgs<T> a)
 {
+    if (a.pdl_early) pdl_trigger();
+    pdl_wait();
     const int sel = chain_sel(a);
     if (sel < 0) return;
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
@@ -261,6 +270,7 @@ __device__ __forceinline__ double pair_force(const PedArgs<double> &a, double d2
 template <typename T>
 __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
 {
+    pdl_enter();
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
     // for the binning chain of the next step, which runs beside this step's tail kernel: go / no go
     if (d == 0) a.ctl->occ_next = a.ctl->halt ? -1 : (a.ctl->parity ^ 1);
@@ -396,6 +406,7 @@ __device__ __forceinline__ double hydrograph(const double *t, const double *q, i
 template <typename T>
 __global__ void tail_kernel(TailArgs<T> a, int first)
 {
+    pdl_enter();
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     Ctl *c = a.ctl;
     if (!first) {
