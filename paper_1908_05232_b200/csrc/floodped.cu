@@ -272,13 +272,13 @@ struct Marks {                                        // profiling mode only: an
 // (B)+(O) of the step that comes NEXT: count -> scan -> scatter -> N_p per cell.  It needs the
 // pedestrians of that step only, so in graph mode it runs beside the flood kernel of the step
 // before (pipelined = 1: it fills the N_p buffer the flood kernel is not reading).
-template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelined, Marks &mark)
+template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelined, Marks &mark, bool counted = false)
 {
     PedArgs<T> pa = ped_args_full<T>(s, pipelined);
     const int nb = (s->np + 255) / 256, n_items = s->nbins + 1;
     const bool pdl = s->pdl && !mark.ev;              // graph mode: each kernel may start under the tail of the one before
     mark();
-    CU(launch_pdl(ped_bin_count_kernel<T>, dim3(nb), dim3(256), 0, st, pdl && pipelined, pa, 1));
+    if (!counted) CU(launch_pdl(ped_bin_count_kernel<T>, dim3(nb), dim3(256), 0, st, pdl && pipelined, pa, 1));
     mark();
     CU(launch_pdl(scan_bins_kernel, dim3((n_items + SCAN_TILE - 1) / SCAN_TILE), dim3(SCAN_THREADS), 0, st, pdl,
                   s->count, s->start, n_items, s->scan_status, s->ctl, pipelined, pa.pdl_early));
@@ -326,7 +326,7 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cuda
             else CU(cudaStreamWaitEvent(sp, s->ev_tail, 0));
         }
         mark();
-        CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + 127) / 128), dim3(128), 0, sp, s->pdl && !ev, ped_args_full<T>(s, 0)));
+        CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + 127) / 128), dim3(128), 0, sp, s->pdl && !ev, ped_args_full<T>(s, 0), fork ? 1 : 0));
         if (fork) {
             CU(cudaEventRecord(s->ev_ped, sp));
             if (!first) CU(cudaStreamWaitEvent(st, s->ev_occ, 0));     // N_p of this step, filled beside the step before
@@ -335,7 +335,7 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cuda
     mark();
     launch_flood<T>(s, st, s->pdl && !ev);
     if (fork) {
-        int rc = enqueue_bin_chain<T>(s, sp, 1, mark);
+        int rc = enqueue_bin_chain<T>(s, sp, 1, mark, true);             // counted inside ped_step
         if (rc != SIM_OK) return rc;
         CU(cudaEventRecord(s->ev_occ, sp));
         CU(cudaStreamWaitEvent(st, s->ev_ped, 0));
@@ -673,7 +673,7 @@ extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
     return DISPATCH(s, step_profiled, s, n, kernel_ms);
 }
 
-extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? 7 : 2) : 0; }
+extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? (s->overlap ? 6 : 7) : 2) : 0; }
 
 extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
 {

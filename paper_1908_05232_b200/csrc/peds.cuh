@@ -67,14 +67,8 @@ template <typename T> __device__ __forceinline__ int cell_of(T x, T inv, int n)
 // order), so lanes of a warp mostly share a key: one atomic per distinct key per warp
 // (warp-aggregated atomics via match.any).  Also clears the occupancy set by the previous step.
 template <typename T>
-__global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int clear_occ)
+__device__ __forceinline__ void bin_count_one(const PedArgs<T> &a, const int s, const int sel, const int clear_occ)
 {
-    if (a.pdl_early) pdl_trigger();
-    pdl_wait();
-    const int sel = chain_sel(a);
-    if (sel < 0) return;
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= a.n) return;
     const unsigned lanes = __activemask();
     int key = a.nbins, cell = -1;
     if (a.A.active[s]) {
@@ -94,6 +88,18 @@ __global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int cl
         const int c = a.cellprev[sel * a.cellprev_stride + s];
         if (c >= 0) a.occ[sel * a.occ_stride + c] = 0;      // sparse clear: only cells that were set (no dense memset)
     }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) ped_bin_count_kernel(PedArgs<T> a, int clear_occ)
+{
+    if (a.pdl_early) pdl_trigger();
+    pdl_wait();
+    const int sel = chain_sel(a);
+    if (sel < 0) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= a.n) return;
+    bin_count_one(a, s, sel, clear_occ);
 }
 
 // ---------------------------------------------------------------------------------- (B) scan
@@ -268,14 +274,8 @@ __device__ __forceinline__ double pair_force(const PedArgs<double> &a, double d2
 // One thread per sorted slot d: reads level n from B (+ flood level n), writes level n+1 to A[d].
 // Independent of the flood kernel of the same step (both read level n), so the two may overlap.
 template <typename T>
-__global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
+__device__ __forceinline__ void ped_step_one(const PedArgs<T> &a, const int d)
 {
-    pdl_enter();
-    const int d = blockIdx.x * blockDim.x + threadIdx.x;
-    // for the binning chain of the next step, which runs beside this step's tail kernel: go / no go
-    if (d == 0) a.ctl->occ_next = a.ctl->halt ? -1 : (a.ctl->parity ^ 1);
-    if (a.ctl->halt) return;
-    if (d >= a.n) return;
     const PedSoA<T> &B = a.B, &A = a.A;
     const T x = B.x[d], y = B.y[d], vx = B.vx[d], vy = B.vy[d], vpref = B.vpref[d];
     T timer = B.timer[d];
@@ -377,6 +377,25 @@ __global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a)
     }
     A.x[d] = xn; A.y[d] = yn; A.vx[d] = wx; A.vy[d] = wy; A.timer[d] = timer;
     A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 1;
+}
+
+
+// fuse_count = 1 (step graph): every thread goes on to key and count its own agent for the binning
+// chain of the NEXT step (the first kernel of that chain folded in: one launch fewer on the
+// critical path of small crowds).  The chain fills N_p buffer parity ^ 1, which the flood kernel
+// running beside this one does not read.
+template <typename T>
+__global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a, int fuse_count)
+{
+    pdl_enter();
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    const int halt = a.ctl->halt, sel = a.ctl->parity ^ 1;
+    // for the binning chain of the next step, which runs beside this step's tail kernel: go / no go
+    if (d == 0) a.ctl->occ_next = halt ? -1 : sel;
+    if (halt) return;
+    if (d >= a.n) return;
+    ped_step_one(a, d);
+    if (fuse_count) bin_count_one(a, d, sel, 1);
 }
 
 // ---------------------------------------------------------------------------------- (S)+(T) tail
