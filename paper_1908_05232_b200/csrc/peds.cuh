@@ -421,39 +421,75 @@ __device__ __forceinline__ double hydrograph(const double *t, const double *q, i
     return q[n - 1];
 }
 
-// first = 1: only derive dt and q_in from the state already in place (create / test hooks)
+// hydrograph() with the table spread over the lanes of a warp: all entries are loaded at once
+// (one memory latency instead of one per segment -- this kernel sits on the critical path of every
+// step).  Same segments, same interpolation expression.  All 32 lanes must call it.
+__device__ __forceinline__ double hydrograph_warp(const double *t, const double *q, int n, double time)
+{
+    if (n <= 0) return 0.0;
+    const int lane = threadIdx.x & 31;
+    double res = 0.0;
+    bool found = false;
+    if (time <= t[0]) { res = q[0]; found = true; }            // warp-uniform
+    for (int base = 0; base + 1 < n && !found; base += 32) {
+        const int k = base + lane;
+        const bool ok = k + 1 < n;
+        const double t0 = ok ? t[k] : 0.0, t1 = ok ? t[k + 1] : 0.0, q0 = ok ? q[k] : 0.0, q1 = ok ? q[k + 1] : 0.0;
+        const unsigned hit = __ballot_sync(0xffffffffu, ok && time < t1);
+        if (hit) {
+            const int src = __ffs(hit) - 1;
+            const double v = q0 + (q1 - q0) * (time - t0) / (t1 - t0);
+            res = __shfl_sync(0xffffffffu, v, src);
+            found = true;
+        }
+    }
+    if (!found) res = q[n - 1];
+    return res;
+}
+
+// first = 1: only derive dt and q_in from the state already in place (create / test hooks).
+// One warp; lane 0 owns the control block.  It works on a register copy read with independent
+// loads and writes back only the fields this kernel owns: the binning chain of the next step may
+// be running beside it and owns scan_ticket / scan_epoch / occ_next.
 template <typename T>
 __global__ void tail_kernel(TailArgs<T> a, int first)
 {
     pdl_enter();
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
     Ctl *c = a.ctl;
+    Ctl l = *c;
+    if (!first && l.halt) return;                              // warp-uniform
     if (!first) {
-        if (c->halt) return;
-        const int D = c->D;
-        c->deposits += D;
-        for (int d = 0; d < D && !c->complete; ++d) {
-            c->bags += 1;
-            if (c->bags == a.bags_per_cell_layer) {
-                a.zs[a.line_cells[c->cursor]] += a.layer_thickness;
-                c->bags = 0; c->cursor += 1;
-                if (c->cursor == a.n_line) { c->layer += 1; c->cursor = 0; }
-                if (c->layer == a.n_layers) c->complete = 1;
+        if (threadIdx.x == 0 && l.D > 0) {                     // deposits of this step
+            const int D = l.D;
+            l.deposits += D;
+            for (int d = 0; d < D && !l.complete; ++d) {
+                l.bags += 1;
+                if (l.bags == a.bags_per_cell_layer) {
+                    a.zs[a.line_cells[l.cursor]] += a.layer_thickness;
+                    l.bags = 0; l.cursor += 1;
+                    if (l.cursor == a.n_line) { l.layer += 1; l.cursor = 0; }
+                    if (l.layer == a.n_layers) l.complete = 1;
+                }
             }
+            c->deposits = l.deposits; c->bags = l.bags; c->cursor = l.cursor; c->layer = l.layer; c->complete = l.complete;
         }
-        c->D = 0;
-        c->t += c->dt;
-        c->step += 1;
-        c->parity ^= 1;
+        l.t += l.dt;
+        l.step += 1;
+        l.parity ^= 1;
     }
-    const double lam = __longlong_as_double((long long)c->lam_bits);
-    double dt = c->dt_max;
-    if (lam > 0.0) dt = fmin(dt, c->cfl / lam);
-    if (c->t + dt > c->t_end) dt = fmax(0.0, c->t_end - c->t);
-    c->dt = dt;
-    c->lam_bits = 0ull;
-    c->halt = (c->t >= c->t_end) ? 1 : 0;
-    c->q_in = hydrograph(a.hydro_t, a.hydro_q, a.n_hydro, c->t) * a.inv_inflow_length;
+    const double lam = __longlong_as_double((long long)l.lam_bits);
+    double dt = l.dt_max;
+    if (lam > 0.0) dt = fmin(dt, l.cfl / lam);
+    if (l.t + dt > l.t_end) dt = fmax(0.0, l.t_end - l.t);
+    const double q_in = hydrograph_warp(a.hydro_t, a.hydro_q, a.n_hydro, l.t) * a.inv_inflow_length;
+    if (threadIdx.x == 0) {
+        if (!first) { c->D = 0; c->t = l.t; c->step = l.step; c->parity = l.parity; }
+        c->dt = dt;
+        c->lam_bits = 0ull;
+        c->halt = (l.t >= l.t_end) ? 1 : 0;
+        c->q_in = q_in;
+    }
 }
 
 // ---------------------------------------------------------------------------------- read-back
