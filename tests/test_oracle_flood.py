@@ -48,6 +48,23 @@ def test_riemann_consistency_and_mirror():
         assert np.allclose([A[0], A[1], A[2]], [-B[0], B[1], -B[2]], rtol=1e-12, atol=1e-12)
 
 
+def test_slip_and_no_slip_walls_give_the_same_flux():
+    """P:L180 names "slip" and "wall" boundaries.  At a mirror ghost (h, -u_n, .) the mass flux is
+    zero, so the tangential momentum flux (mass flux x upwind tangential velocity) is zero whatever
+    tangential velocity the ghost carries: free-slip (+v), no-slip (-v) or anything else give the
+    same three fluxes, and the normal one is the wall pressure (reading C13)."""
+    rng = np.random.default_rng(17)
+    for _ in range(200):
+        h, u, v = rng.uniform(0.01, 3), rng.uniform(-4, 4), rng.uniform(-2, 2)
+        slip = oracle.riemann_flux(G, h, u, v, h, -u, v)
+        noslip = oracle.riemann_flux(G, h, u, v, h, -u, -v)
+        other = oracle.riemann_flux(G, h, u, v, h, -u, rng.uniform(-5, 5))
+        for F in (slip, noslip, other):
+            assert abs(F[0]) <= 1e-13 * h * (abs(u) + np.sqrt(G * h)) and abs(F[2]) <= 1e-12
+            assert F[1] == pytest.approx(slip[1], rel=1e-13)
+        assert slip[1] >= 0.5 * G * h * h * (1 - 1e-12) if u >= 0 else slip[1] <= 0.5 * G * h * h * (1 + 1e-12)
+
+
 # ------------------------------------------------------------------ C-property (BJ north_star)
 
 @pytest.mark.parametrize("eta", [0.5, 0.2])          # 0.2 < bump top 0.3: an island emerges
