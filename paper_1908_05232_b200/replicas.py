@@ -95,7 +95,7 @@ def barrier_sweep_items(layers=(1, 2, 3, 4, 5, 6), shares=(0.05, 0.10, 0.20, 0.3
 
 
 def run_barrier_item(item: dict, n: int = 128, n_people: int = 400, t_end: float = 600.0, device="cuda:0",
-                     t_release: float = 120.0, steps_per_poll: int = 256) -> dict:
+                     t_release: float = 120.0, steps_per_poll: int = 32) -> dict:
     """One run of the pre-flood intervention on the synthetic hall (Config 3 recipe at n x n):
     `share` of the people are responders who build `n_layers` layers of the barrier line, the
     flood is released at `t_release`.  Returns the quantities of the paper's Figs 8-10:
