@@ -205,3 +205,25 @@ def test_rows_per_chunk_do_not_change_the_flood():
     for o in outs[1:]:
         for k in ("h", "qx", "qy"):
             assert mixed(o[k], outs[0][k]) <= 6 * 2e-6, (k, mixed(o[k], outs[0][k]))
+
+
+def test_long_hydrograph_table_is_interpolated_like_the_oracle():
+    """70 break points (more than one warp of table entries in the tail kernel), times landing
+    before, inside and after the table"""
+    n = 64
+    rng = np.random.default_rng(21)
+    ht = np.cumsum(rng.uniform(0.05, 0.4, 70)) + 0.3
+    hq = rng.uniform(0.0, 6.0, 70)
+    sc = box(n, n, dx=0.5, real_bits=64, h0=0.05, manning=0.02, dt_max=0.25,
+             inflow_cell=np.arange(10, 30, dtype=np.int32), inflow_side=np.full(20, S.SIDE_S, np.uint8),
+             hydro_t=ht, hydro_q=hq)
+    o, g = make_pair(sc)
+    for _ in range(30):
+        o.step(7); g.step(7)
+        so, sg = o.stats(), g.stats()
+        assert sg["t"] == pytest.approx(so["t"], rel=1e-12)
+        assert sg["volume"] == pytest.approx(so["volume"], rel=1e-11)
+    assert o.stats()["t"] > ht[-1]                          # ran past the end of the table
+    a, b = g.read_conserved(), o.read_conserved()
+    for k in ("h", "qx", "qy"):
+        assert mixed(a[k], b[k]) <= 1e-9, k
