@@ -31,7 +31,9 @@ struct FloodArgs {
     const uint8_t *occ;               // N_p per cell (saturated at 255): buffer 0; the step at flood parity p reads occ + p * occ_stride
     size_t occ_stride;
     const uint8_t *inflow[4];         // per edge cell: number of inflow faces on that side (W,E,S,N)
-    const uint8_t *chunk_flag;        // march kernel: 1 = chunk takes the general path (flood_march.cuh)
+    const uint8_t *chunk_flag;        // march kernels: path of every chunk (flood_chunk_flags_kernel)
+    const T *ghost_zero, *ghost_inf;  // one strip-wide row of zeros / of +inf, and of zero bytes: the row beyond the
+    const uint8_t *ghost_occ;         // domain edge as the TMA kernel loads it (a wall = a row of solid cells, C13)
     int R;                            // march kernel: rows per chunk
     Ctl *ctl;
 };

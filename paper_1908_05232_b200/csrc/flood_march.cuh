@@ -248,8 +248,9 @@ __global__ void __launch_bounds__(MW, sizeof(T) == 4 ? 4 : 2) flood_march_kernel
     }
 }
 
-// Which path a chunk takes: 1 = it touches the domain edge (general path: bounds checks, wall
-// ghosts, inflow); 2 = interior, but a solid cell lies in it or in its one-cell halo (the row-marching
+// Which path a chunk takes: 1 = it touches the domain edge and its strip sticks out of the domain
+// (general path: bounds checks, wall ghosts, inflow); 3 = it touches the domain edge, strip inside
+// (variant 4: TMA path with ghost rows; variants 2 and 3 treat it like 1); 2 = interior, but a solid cell lies in it or in its one-cell halo (the row-marching
 // kernels with wall-ghost selects; variants 2 and 3 treat it like 1); 0 = interior, no solid.
 // One CTA per chunk; rerun whenever the bed array is rewritten.
 template <typename T>
@@ -266,7 +267,7 @@ __global__ void flood_chunk_flags_kernel(const T *__restrict__ zs, int nx, int n
         }
     }
     solid = __syncthreads_or(solid);
-    if (threadIdx.x == 0) flag[blockIdx.y * gridDim.x + blockIdx.x] = (uint8_t)(edge ? 1 : solid ? 2 : 0);
+    if (threadIdx.x == 0) flag[blockIdx.y * gridDim.x + blockIdx.x] = (uint8_t)(edge ? (x0 + MW <= nx ? 3 : 1) : solid ? 2 : 0);
 }
 
 }  // namespace fp

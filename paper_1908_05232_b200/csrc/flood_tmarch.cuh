@@ -14,8 +14,10 @@
 //   registers by then).
 //
 //   chunk_flag picks the path of a chunk: 0 = interior without solid cells (no selects), 2 = interior
-//   with solid cells in it or its halo (same path with wall-ghost selects, SOLID = true), 1 = touching
-//   the domain edge (march2_chunk<GEN=true>: plain loads, bounds checks, inflow).
+//   with solid cells in it or its halo (same path with wall-ghost selects, SOLID = true), 3 = touching
+//   the domain edge with the strip inside the domain (EDGE = true: ghost rows of solid cells beyond the
+//   edge, inflow faces, a short last chunk), 1 = edge chunk of a strip that sticks out of the domain
+//   (march2_chunk<GEN=true>: plain loads, bounds checks, inflow).
 //   Needs nx % 16 == 0 (16-byte alignment of every row segment).
 //
 //   TM_SPLIT_BARRIER=1 builds the measured-and-dropped alternative to the per-row __syncthreads: a
@@ -77,14 +79,24 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// one row segment (columns x0 .. x0+MW-1 of row j) -> stage
-template <typename T>
+// one row segment (columns x0 .. x0+MW-1 of row j) -> stage; EDGE: a row beyond the domain is the
+// ghost row of solid cells (the wall, C13)
+template <typename T, bool EDGE>
 __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, const T *QX, const T *QY, const uint8_t *OCC,
                                              RowStage<T> &st, uint64_t *bar, int x0, int j)
 {
-    const size_t c = (size_t)j * a.nx + x0;
     constexpr uint32_t RB = MW * sizeof(T);
     mbar_expect_tx(bar, 5 * RB + MW);
+    if (EDGE && (j < 0 || j >= a.ny)) {
+        bulk_g2s(st.h, a.ghost_zero, RB, bar);
+        bulk_g2s(st.qx, a.ghost_zero, RB, bar);
+        bulk_g2s(st.qy, a.ghost_zero, RB, bar);
+        bulk_g2s(st.z, a.ghost_inf, RB, bar);
+        bulk_g2s(st.n0, a.ghost_zero, RB, bar);
+        bulk_g2s(st.occ, a.ghost_occ, MW, bar);
+        return;
+    }
+    const size_t c = (size_t)j * a.nx + x0;
     bulk_g2s(st.h, H + c, RB, bar);
     bulk_g2s(st.qx, QX + c, RB, bar);
     bulk_g2s(st.qy, QY + c, RB, bar);
@@ -93,17 +105,22 @@ __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, 
     bulk_g2s(st.occ, OCC + c, MW, bar);
 }
 
-// interior chunk (no domain edge; SOLID: solid cells in it or in its halo): rows y0-1 .. y0+R all exist
+// one chunk.  SOLID: solid cells in it or in its halo (wall-ghost selects).  EDGE (implies SOLID): it
+// touches the domain edge: rows and columns beyond it are ghost solid cells, inflow faces add their
+// discharge (C14), the last chunk of a strip may be shorter than R.
 //
 //   Synchronisation per row: the neighbour exchange (last-column state st[b], west-face flux
 //   fx[b]) needs one CTA-wide barrier per row.  It sits AFTER the south faces, which need nothing
 //   from the neighbours, so the skew between warps is spent on useful work first.  The ring slot is
 //   refilled after that barrier (all threads have their values in registers by then).  The TMA issue sits in a warp-uniform branch with one elected
 //   lane, its addresses derived from uniform values only.
-template <typename T, int CPT, int STAGES, bool SOLID>
+template <typename T, int CPT, int STAGES, bool SOLID, bool EDGE>
 __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, CPT> &s, RowStage<T> *ring,
-                                          uint64_t *bars, int x0, int y0, int R)
+                                          uint64_t *bars, int x0, int y0, int Rfull)
 {
+    const int R = EDGE ? min(Rfull, a.ny - y0) : Rfull;   // rows of this chunk inside the domain
+    const T qin = EDGE ? (T)a.ctl->q_in : T(0);
+    const int ny = a.ny;
     constexpr int NT = MW / CPT;
     const int tid = threadIdx.x;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);       // warp-uniform by construction
@@ -128,15 +145,15 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     __syncthreads();
     if (warp == 0) {
         if (elect_one())
-            for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row(a, H, QX, QY, OCC, ring[r], &bars[r], x0, y0 - 1 + r);
+            for (int r = 0; r < STAGES && r < nrows; ++r) tm_issue_row<T, EDGE>(a, H, QX, QY, OCC, ring[r], &bars[r], x0, y0 - 1 + r);
     }
 
     // ---- pre-pass: strip-edge data for every row of the chunk (as in variants 2, 3)
     for (int k = tid; k < R; k += NT) {
         const int j = y0 + k;
-        Raw4<T> l = march_load<T, false>(H, QX, QY, Z, x0 + MW - 1, j, nx, a.ny);
-        Raw4<T> r = march_load<T, false>(H, QX, QY, Z, x0 + MW, j, nx, a.ny);
-        Raw4<T> w = march_load<T, false>(H, QX, QY, Z, x0 - 1, j, nx, a.ny);
+        Raw4<T> l = march_load<T, EDGE>(H, QX, QY, Z, x0 + MW - 1, j, nx, a.ny);
+        Raw4<T> r = march_load<T, EDGE>(H, QX, QY, Z, x0 + MW, j, nx, a.ny);
+        Raw4<T> w = march_load<T, EDGE>(H, QX, QY, Z, x0 - 1, j, nx, a.ny);
         T el, ul, vl, er_, ur, vr, ew, uw, vw, f0, f1L, f1R, f2;
         march_prims<T, SOLID>(l, h_dry, el, ul, vl);
         march_prims<T, SOLID>(r, h_dry, er_, ur, vr);
@@ -164,7 +181,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
     }
     __syncthreads();                                   // slot 0 consumed; er/sw visible
     if (warp == 0 && STAGES < nrows) {
-        if (elect_one()) tm_issue_row(a, H, QX, QY, OCC, ring[0], &bars[0], x0, y0 - 1 + STAGES);
+        if (elect_one()) tm_issue_row<T, EDGE>(a, H, QX, QY, OCC, ring[0], &bars[0], x0, y0 - 1 + STAGES);
     }
 
     T ah[CPT], ax[CPT], ay[CPT], n0_p[CPT];
@@ -233,7 +250,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         __syncthreads();                               // st[b] of this row and fx[b^1] of the previous one are visible
 #endif
         if (warp == 0 && it + 1 + STAGES < nrows) {
-            if (elect_one()) tm_issue_row(a, H, QX, QY, OCC, ring[slot], tbar, x0, y0 + it + STAGES);
+            if (elect_one()) tm_issue_row<T, EDGE>(a, H, QX, QY, OCC, ring[slot], tbar, x0, y0 + it + STAGES);
         }
         sp += sizeof(RowStage<float>); op += sizeof(RowStage<float>); tbar += 1;
         if (++slot == STAGES) {
@@ -252,7 +269,8 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
             for (int k = 0; k < NP; ++k)
                 bits |= __float_as_uint(g0[k].x) | __float_as_uint(g0[k].y) | __float_as_uint(g1L[k].x) | __float_as_uint(g1L[k].y)
                       | __float_as_uint(g2[k].x) | __float_as_uint(g2[k].y);
-            const bool live = live_p || (bits << 1) != 0u;
+            const int jrow = y0 + it - 1;
+            const bool live = live_p || (bits << 1) != 0u || (EDGE && (jrow == ny - 1 || i + CPT == nx));
             VecN<f2, NP> ho, qxo, qyo;
 #pragma unroll
             for (int k = 0; k < NP; ++k) ho.v[k] = qxo.v[k] = qyo.v[k] = pk1(0.f);
@@ -263,6 +281,16 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 }
                 ho.v[NP - 1].y = fmaf(-dtdx, e0, ho.v[NP - 1].y); qxo.v[NP - 1].y = fmaf(-dtdx, e1, qxo.v[NP - 1].y);
                 qyo.v[NP - 1].y = fmaf(-dtdx, e2, qyo.v[NP - 1].y);
+                if (EDGE) {                            // inflow faces on the east / north edge (C14)
+                    if (i + CPT == nx) ho.v[NP - 1].y += dtdx * qin * float(a.inflow[1][jrow]);
+                    if (jrow == ny - 1) {
+#pragma unroll
+                        for (int k = 0; k < NP; ++k) {
+                            ho.v[k].x += dtdy * qin * float(a.inflow[3][i + 2 * k]);
+                            ho.v[k].y += dtdy * qin * float(a.inflow[3][i + 2 * k + 1]);
+                        }
+                    }
+                }
                 if (SOLID) {                           // nothing moves in a solid cell (and no clamp is counted)
 #pragma unroll
                     for (int k = 0; k < NP; ++k) {
@@ -307,6 +335,13 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 } else {                               // east face of the first column; the second one's comes from the neighbour
                     ah2[k].x = fmaf(-dtdx, f0[k].y, ah2[k].x); ax2[k].x = fmaf(-dtdx, f1L[k].y, ax2[k].x);
                     ay2[k].x = fmaf(-dtdx, f2v[k].y, ay2[k].x);
+                }
+                if (EDGE) {                            // inflow faces on the west / south edge (C14)
+                    if (k == 0 && i == 0) ah2[0].x += dtdx * qin * float(a.inflow[0][y0 + it]);
+                    if (y0 + it == 0) {
+                        ah2[k].x += dtdy * qin * float(a.inflow[2][i + 2 * k]);
+                        ah2[k].y += dtdy * qin * float(a.inflow[2][i + 2 * k + 1]);
+                    }
                 }
                 ab |= __float_as_uint(ah2[k].x) | __float_as_uint(ah2[k].y) | __float_as_uint(ax2[k].x)
                     | __float_as_uint(ax2[k].y) | __float_as_uint(ay2[k].x) | __float_as_uint(ay2[k].y);
@@ -362,7 +397,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
         __syncthreads();                               // st[b] of this row and fx[b^1] of the previous one are visible
 #endif
         if (warp == 0 && it + 1 + STAGES < nrows) {
-            if (elect_one()) tm_issue_row(a, H, QX, QY, OCC, ring[slot], tbar, x0, y0 + it + STAGES);
+            if (elect_one()) tm_issue_row<T, EDGE>(a, H, QX, QY, OCC, ring[slot], tbar, x0, y0 + it + STAGES);
         }
         sp += sizeof(RowStage<T>); op += sizeof(RowStage<T>); tbar += 1;
         if (++slot == STAGES) {
@@ -375,7 +410,7 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
             const int stride = last_thread ? MARCH_MAX_R : NT;
             const T e0 = fe[0], e1 = fe[stride], e2 = fe[2 * stride];
             // a warp whose cells of this row hold exact zeros and receive no flux writes zeros
-            bool live = live_p || e0 != T(0) || e1 != T(0) || e2 != T(0);
+            bool live = live_p || e0 != T(0) || e1 != T(0) || e2 != T(0) || (EDGE && (y0 + it - 1 == ny - 1 || i + CPT == nx));
 #pragma unroll
             for (int k = 0; k < CPT; ++k) live = live || g0[k] != T(0) || g1L[k] != T(0) || g2[k] != T(0);
             VecN<T, CPT> ho, qxo, qyo;
@@ -386,6 +421,8 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 for (int k = 0; k < CPT; ++k) {
                     T hn = ah[k] - dtdy * g0[k], qxn = ax[k] - dtdy * g2[k], qyn = ay[k] - dtdy * g1L[k];
                     if (k == CPT - 1) { hn -= dtdx * e0; qxn -= dtdx * e1; qyn -= dtdx * e2; }
+                    if (EDGE && k == CPT - 1 && i + CPT == nx) hn += dtdx * qin * T(a.inflow[1][y0 + it - 1]);
+                    if (EDGE && y0 + it - 1 == ny - 1) hn += dtdy * qin * T(a.inflow[3][i + k]);
                     if (SOLID && is_solid(z_p[k])) { hn = qxn = qyn = T(0); }
                     finish_hat2(a, dt, hn, qxn, qyn, n0_p[k], occ_p[k], lam, clamp_h, clamp_n);
                     ho.v[k] = hn; qxo.v[k] = qxn; qyo.v[k] = qyn;
@@ -415,6 +452,8 @@ __device__ __forceinline__ T tmarch_chunk(const FloodArgs<T> &a, March2Smem<T, C
                 ax[k] = qxc[k] + dtdx * f1R[k] + dtdy * g2[k];
                 ay[k] = qyc[k] + dtdx * f2[k] + dtdy * g1R[k];
                 if (k < CPT - 1) { ah[k] -= dtdx * f0[k + 1]; ax[k] -= dtdx * f1L[k + 1]; ay[k] -= dtdx * f2[k + 1]; }
+                if (EDGE && i + k == 0) ah[k] += dtdx * qin * T(a.inflow[0][y0 + it]);
+                if (EDGE && y0 + it == 0) ah[k] += dtdy * qin * T(a.inflow[2][i + k]);
                 live_p = live_p || ah[k] != T(0) || ax[k] != T(0) || ay[k] != T(0);
             }
         }
@@ -453,8 +492,9 @@ __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tma
     const int x0 = blockIdx.x * MW, y0 = blockIdx.y * a.R;
     const int path = a.chunk_flag[blockIdx.y * gridDim.x + blockIdx.x];
     T lam = path == 1 ? march2_chunk<T, CPT, true>(a, s, x0, y0, a.R)
-          : path == 2 ? tmarch_chunk<T, CPT, STAGES, true>(a, s, ring, bars, x0, y0, a.R)
-                      : tmarch_chunk<T, CPT, STAGES, false>(a, s, ring, bars, x0, y0, a.R);
+          : path == 3 ? tmarch_chunk<T, CPT, STAGES, true, true>(a, s, ring, bars, x0, y0, a.R)
+          : path == 2 ? tmarch_chunk<T, CPT, STAGES, true, false>(a, s, ring, bars, x0, y0, a.R)
+                      : tmarch_chunk<T, CPT, STAGES, false, false>(a, s, ring, bars, x0, y0, a.R);
     const int tid = threadIdx.x;
     for (int o = 16; o > 0; o >>= 1) lam = fmax(lam, __shfl_xor_sync(0xffffffffu, lam, o));
     __syncthreads();

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <limits>
 #include <cstdlib>
 #include <string>
 #include <vector>
@@ -63,6 +64,7 @@ struct sim {
     int flood_variant = 1;
     int march_R = 64, march_gx = 1, march_gy = 1;
     uint8_t *chunk_flag = nullptr;
+    void *ghost_zero = nullptr, *ghost_inf = nullptr;   // one strip-wide row each (TMA kernel, rows beyond the domain)
     int exit_i[16]{}, exit_j[16]{};
     cudaGraphExec_t graph1 = nullptr, graphN = nullptr;
     cudaStream_t stream2 = nullptr;   // second branch of the step graph (pedestrian step beside the flood step)
@@ -120,6 +122,7 @@ size_t layout(sim *s, Bump &b)
     s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(2 * np);
     s->bxy = real(2 * (size_t)np);
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
+    s->ghost_zero = b.take<double>(MW); s->ghost_inf = b.take<double>(MW);
     s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * ((s->grid.ny + 7) / 8));    // room for any R >= 8
     s->scan_status = b.take<unsigned long long>((size_t)(s->nbins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1);
     return (b.off + 255) & ~size_t(255);
@@ -197,6 +200,7 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     a.zs = (const T *)s->zs; a.n0 = (const T *)s->n0; a.occ = s->occ; a.occ_stride = (size_t)s->ncell;
     for (int k = 0; k < 4; ++k) a.inflow[k] = s->inflow[k];
     a.chunk_flag = s->chunk_flag; a.R = s->march_R;
+    a.ghost_zero = (const T *)s->ghost_zero; a.ghost_inf = (const T *)s->ghost_inf; a.ghost_occ = (const uint8_t *)s->ghost_zero;
     a.ctl = s->ctl;
     return a;
 }
@@ -453,6 +457,8 @@ int upload(sim *s, void *dst, const void *src, size_t bytes)
 }
 
 // host-side preparation of one real array with solids applied
+template <typename T> T solid_value() { return std::numeric_limits<T>::infinity(); }
+
 template <typename T>
 void make_zs(const T *z, const uint8_t *mask, size_t n, std::vector<T> &out)
 {
@@ -486,6 +492,11 @@ int upload_state(sim *s, const sim_topo_t *topo, const void *manning, const sim_
     make_zs<T>((const T *)topo->z, topo->mask, nc, tmp);
     if (upload(s, s->zs, tmp.data(), nc * rs)) return SIM_ECUDA;
     CU(cudaStreamSynchronize(s->stream));
+    {   // the row beyond the domain edge: solid cells (ghost_zero stays at the workspace's zeros)
+        std::vector<T> inf(MW, solid_value<T>());
+        if (upload(s, s->ghost_inf, inf.data(), MW * rs)) return SIM_ECUDA;
+        CU(cudaStreamSynchronize(s->stream));
+    }
     if (upload(s, s->z0, topo->z, nc * rs)) return SIM_ECUDA;
     if (upload(s, s->n0, manning, nc * rs)) return SIM_ECUDA;
     if (upload(s, s->mask, topo->mask, nc)) return SIM_ECUDA;
