@@ -35,7 +35,7 @@ FLOOD_BYTES_PER_CELL = 33        # fp32: read h,qx,qy,z,n0 (20) + N_p (1) ; writ
 PED_BYTES_PER_AGENT = 175        # key+count 17, scatter 72, step 85
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the flood kernel, from the committed
 # ncu --set full capture (profiles/r1_final_ncu_full_c5.md); only for the exact workload profiled
-NCU_TRAFFIC_BYTES = {(5, 4): 1.581725e9 + 770.959e6}
+NCU_TRAFFIC_BYTES = {(5, 4): 1.588444e9 + 770.069e6}
 
 
 def peaks():
