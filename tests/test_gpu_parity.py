@@ -119,7 +119,8 @@ def test_config4_mini_single_step_fp32_buildings_all_hr_classes(variant):
     assert hist[1] > 0 and hist[2] > 0 and hist[3] > 0      # low, medium, high all present
 
 
-@pytest.mark.parametrize("nx,ny", [(4, 4), (64, 16), (100, 37), (130, 50), (33, 9), (7, 5), (300, 70), (257, 33), (512, 130)])
+@pytest.mark.parametrize("nx,ny", [(4, 4), (64, 16), (100, 37), (130, 50), (33, 9), (7, 5), (300, 70), (257, 33), (512, 130),
+                                   (256, 24), (768, 19), (512, 9), (1024, 8), (272, 40)])
 def test_ragged_tiles_and_tiny_grids(nx, ny):
     rng = np.random.default_rng(nx * 100 + ny)
     z = 0.2 * rng.random((ny, nx))
