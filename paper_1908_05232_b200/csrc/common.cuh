@@ -26,6 +26,8 @@ struct Ctl {
     unsigned int scan_epoch;         // makes the look-back flags of the scan self-resetting
     unsigned int scan_ticket;        // dynamic tile index of the scan
     int occ_next;                    // N_p buffer the binning chain of the NEXT step fills (= parity ^ 1), published by the pedestrian step
+    float pair_c1, pair_c2;          // fp32 pair force A_s e^{(2r-d)/B_s} = 2^{c1 + c2 d}: read from memory once per thread so that they
+                                     // stay in registers (as kernel parameters ptxas reloads them from the constant bank per candidate)
 };
 
 template <typename T> struct Vec4 { T v[4]; };

@@ -23,7 +23,7 @@ namespace {
 
 thread_local std::string g_create_error;
 
-constexpr int GRAPH_CHUNK = 32;     // coupled steps per large graph launch
+constexpr int GRAPH_LEVELS = 7;     // step graphs of 1, 2, 4, ... 64 coupled steps: any n is a few gap-free replays
 
 struct Bump {                       // carve device state out of one workspace
     char *base = nullptr; size_t off = 0, cap = 0; bool dry = true;
@@ -66,7 +66,9 @@ struct sim {
     uint8_t *chunk_flag = nullptr;
     void *ghost_zero = nullptr, *ghost_inf = nullptr;   // one strip-wide row each (TMA kernel, rows beyond the domain)
     int exit_i[16]{}, exit_j[16]{};
-    cudaGraphExec_t graph1 = nullptr, graphN = nullptr;
+    cudaGraphExec_t graph[GRAPH_LEVELS]{};          // graph[k] advances 2^k coupled steps; built on first use
+    int device = 0;                   // the device the handle lives on; every entry point runs on it
+    int n_sm = 148;
     cudaStream_t stream2 = nullptr;   // second branch of the step graph (pedestrian step beside the flood step)
     cudaEvent_t ev_fork = nullptr, ev_ped = nullptr, ev_occ = nullptr, ev_tail = nullptr;
     int overlap = 1;
@@ -329,7 +331,7 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cuda
             else CU(cudaStreamWaitEvent(sp, s->ev_tail, 0));
         }
         mark();
-        CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + 127) / 128), dim3(128), 0, sp, s->pdl && !ev, ped_args_full<T>(s, 0), fork ? 1 : 0));
+        CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + PED_THREADS - 1) / PED_THREADS), dim3(PED_THREADS), 0, sp, s->pdl && !ev, ped_args_full<T>(s, 0), fork ? 1 : 0));
         if (fork) {
             CU(cudaEventRecord(s->ev_ped, sp));
             if (!first) CU(cudaStreamWaitEvent(st, s->ev_occ, 0));     // N_p of this step, filled beside the step before
@@ -397,30 +399,26 @@ template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
 
 void drop_graphs(sim *s)
 {
-    if (s->graph1) cudaGraphExecDestroy(s->graph1);
-    if (s->graphN) cudaGraphExecDestroy(s->graphN);
-    s->graph1 = s->graphN = nullptr;
+    for (auto &g : s->graph) { if (g) cudaGraphExecDestroy(g); g = nullptr; }
 }
 
-template <typename T> int build_graphs(sim *s)
+template <typename T> int build_graph(sim *s, int level)
 {
-    for (int which = 0; which < 2; ++which) {
-        const int reps = which ? GRAPH_CHUNK : 1;
-        cudaGraph_t g = nullptr;
-        CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
-        int rc = SIM_OK;
-        for (int r = 0; r < reps && rc == SIM_OK; ++r) rc = enqueue_step<T>(s, s->cap_stream, r == 0);
-        if (rc == SIM_OK && s->np > 0 && s->overlap && cudaStreamWaitEvent(s->cap_stream, s->ev_occ, 0) != cudaSuccess)
-            rc = fail(s, SIM_ECUDA, "graph capture: join");
-        cudaError_t e = cudaStreamEndCapture(s->cap_stream, &g);
-        if (rc != SIM_OK) { if (g) cudaGraphDestroy(g); return rc; }
-        if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
-        cudaGraphExec_t ex = nullptr;
-        e = cudaGraphInstantiate(&ex, g, 0);
-        cudaGraphDestroy(g);
-        if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
-        (which ? s->graphN : s->graph1) = ex;
-    }
+    const int reps = 1 << level;
+    cudaGraph_t g = nullptr;
+    CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+    int rc = SIM_OK;
+    for (int r = 0; r < reps && rc == SIM_OK; ++r) rc = enqueue_step<T>(s, s->cap_stream, r == 0);
+    if (rc == SIM_OK && s->np > 0 && s->overlap && cudaStreamWaitEvent(s->cap_stream, s->ev_occ, 0) != cudaSuccess)
+        rc = fail(s, SIM_ECUDA, "graph capture: join");
+    cudaError_t e = cudaStreamEndCapture(s->cap_stream, &g);
+    if (rc != SIM_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+    cudaGraphExec_t ex = nullptr;
+    e = cudaGraphInstantiate(&ex, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
+    s->graph[level] = ex;
     return SIM_OK;
 }
 
@@ -643,6 +641,8 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         c.t = 0.0; c.dt = 0.0; c.t_end = s->prm.t_end; c.dt_max = s->prm.dt_max; c.cfl = s->prm.cfl;
         c.complete = (p->n_line <= 0 || p->n_layers <= 0) ? 1 : 0;
         c.scan_epoch = 1;
+        c.pair_c1 = (float)(2.0 * p->radius / p->B_s * 1.4426950408889634 + std::log2(p->A_s));
+        c.pair_c2 = (float)(-1.4426950408889634 / p->B_s);
         CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         CU(cudaStreamSynchronize(s->stream));
         r = DISPATCH(s, set_smem_attr, s);
@@ -663,16 +663,26 @@ extern "C" int sim_step(sim_t *s, int64_t n)
     if (!s) return SIM_EINVAL;
     if (n < 0) return fail(s, SIM_EINVAL, "negative step count");
     if (n == 0) return SIM_OK;
-    if (!s->graph1) {
-        int rc = DISPATCH(s, build_graphs, s);
-        if (rc != SIM_OK) return rc;
-    }
     {
         int rc = DISPATCH(s, prepare_bins, s);
         if (rc != SIM_OK) return rc;
     }
-    while (n >= GRAPH_CHUNK) { CU(cudaGraphLaunch(s->graphN, s->stream)); n -= GRAPH_CHUNK; }
-    while (n > 0) { CU(cudaGraphLaunch(s->graph1, s->stream)); n -= 1; }
+    // all graphs are captured at the first call (a few ms, once), never inside a later, timed call
+    for (int level = 0; level < GRAPH_LEVELS; ++level)
+        if (!s->graph[level]) {
+            int rc = DISPATCH(s, build_graph, s, level);
+            if (rc != SIM_OK) return rc;
+        }
+    // n = sum of powers of two: the largest graph repeatedly, then one replay per set bit
+    for (int level = GRAPH_LEVELS - 1; level >= 0 && n > 0; --level) {
+        const int64_t reps = (int64_t)1 << level;
+        if (n < reps) continue;
+        while (n >= reps) {
+            CU(cudaGraphLaunch(s->graph[level], s->stream));
+            n -= reps;
+            if (level < GRAPH_LEVELS - 1) break;
+        }
+    }
     return SIM_OK;
 }
 

@@ -256,19 +256,62 @@ __global__ void __launch_bounds__(256) ped_occ_kernel(PedArgs<T> a)
     cellprev[d] = c;
 }
 
-// A_s exp((2r - d)/B_s) / d for the pair at squared distance d2 (C24)
-__device__ __forceinline__ float pair_force(const PedArgs<float> &a, float d2)
+// One candidate of the pair loop: adds A_s exp((2r - d)/B_s) (x_i - x_j)/d to (ax, ay) if 0 < d < R_int
+// (C24, C26).
+//   fp32: the difference and its squares on packed FADD2 / FFMA2; the squares carry +5e-31 each, so
+//   d2 >= 1e-30 > 0 and the agent itself or a coincident partner (d = 0, skipped by C26) needs no
+//   second compare: its force factor is finite and multiplies dx = dy = 0.  Two MUFU (rsqrt, ex2).
+// ---------------------------------------------------------------------------------- (P) pair loop
+// One candidate of the pair loop: adds A_s exp((2r - d)/B_s) (x_i - x_j)/d to (ax, ay) if 0 < d < R_int
+// (C24, C26).
+//   fp32: the difference and its squares on packed FADD2 / FFMA2; the squares carry +5e-31 each, so
+//   d2 >= 1e-30 > 0 and the agent itself or a coincident partner (d = 0, skipped by C26) needs no
+//   second compare: its force factor is finite and multiplies dx = dy = 0.  Two MUFU (rsqrt, ex2);
+//   the force constants are read from memory once per thread (Ctl::pair_c1).  12 instructions per
+//   candidate (16 in round 1).  The kernel stays bound by the XU pipe: a predicated-off MUFU still
+//   occupies it for the whole warp, and two thirds of the candidates of the 3 x 3 bins lie outside
+//   R_int.  Three ways of issuing the MUFU pair only for pairs inside the cut-off were built and
+//   measured on Config 5: all of them cost more issue slots than the XU cycles they save.
+template <typename T> struct PairConst { T R2, c1, c2; };
+template <typename T> __device__ __forceinline__ PairConst<T> pair_const(const PedArgs<T> &a)
 {
-    const float rinv = fast_rsqrt(d2);
-    float e;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fmaf(d2 * rinv, a.c_exp2, a.c_exp1)));
-    return e * rinv;
+    PairConst<T> k{a.R2, a.c_exp1, a.c_exp2};
+    if constexpr (sizeof(T) == 4) { k.c1 = a.ctl->pair_c1; k.c2 = a.ctl->pair_c2; }   // see Ctl
+    return k;
 }
-__device__ __forceinline__ double pair_force(const PedArgs<double> &a, double d2)
+
+__device__ __forceinline__ void pair_add(const PedArgs<float> &, const PairConst<float> &k, float x, float y, VecN<float, 2> pj, float &ax, float &ay)
 {
-    const double d = sqrt(d2);
-    return a.A_s * exp((a.two_r - d) * a.inv_B) / d;
+    const f2 dd = sub2(pk(x, y), pk(pj.v[0], pj.v[1]));
+    const f2 sq = fma2(dd, dd, pk1(5e-31f));
+    const float d2 = sq.x + sq.y;
+    if (d2 < k.R2) {
+        const float rinv = fast_rsqrt(d2);
+        float e;
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fmaf(d2 * rinv, k.c2, k.c1)));
+        const float f = e * rinv;
+        ax = fmaf(f, dd.x, ax); ay = fmaf(f, dd.y, ay);
+    }
 }
+__device__ __forceinline__ void pair_add(const PedArgs<double> &a, const PairConst<double> &, double x, double y, VecN<double, 2> pj, double &ax, double &ay)
+{
+    const double ddx = x - pj.v[0], ddy = y - pj.v[1];
+    const double d2 = ddx * ddx + ddy * ddy;
+    if (d2 > 0.0 && d2 < a.R2) {
+        const double d = sqrt(d2);
+        const double f = a.A_s * exp((a.two_r - d) * a.inv_B) / d;
+        ax += f * ddx; ay += f * ddy;
+    }
+}
+
+#ifndef PED_UNROLL
+#define PED_UNROLL 8
+#endif
+#ifndef PED_THREADS_N
+#define PED_THREADS_N 128
+#endif
+constexpr int PED_THREADS = PED_THREADS_N;
+constexpr int PED_UNROLL_K = PED_UNROLL;
 
 // ---------------------------------------------------------------------------------- (P)+(O)
 // One thread per sorted slot d: reads level n from B (+ flood level n), writes level n+1 to A[d].
@@ -294,18 +337,12 @@ __device__ __forceinline__ void ped_step_one(const PedArgs<T> &a, const int d)
     // 4. social repulsion over the 3 x 3 adjacent bins (C24, C26): three contiguous
     //    index ranges, one per bin row
     T ax = T(0), ay = T(0);
+    const PairConst<T> kc = pair_const(a);
     for (int jy = max(by - 1, 0); jy <= min(by + 1, a.nby - 1); ++jy) {
         const int s0 = a.start[jy * a.nbx + max(bx - 1, 0)];
         const int s1 = a.start[jy * a.nbx + min(bx + 1, a.nbx - 1) + 1];
-        for (int j = s0; j < s1; ++j) {
-            const VecN<T, 2> pj = a.bxy[j];
-            const T ddx = x - pj.v[0], ddy = y - pj.v[1];
-            const T d2 = ddx * ddx + ddy * ddy;
-            if (d2 > T(0) && d2 < a.R2) {
-                const T f = pair_force(a, d2);
-                ax += f * ddx; ay += f * ddy;
-            }
-        }
+#pragma unroll PED_UNROLL_K
+        for (int j = s0; j < s1; ++j) pair_add(a, kc, x, y, a.bxy[j], ax, ay);
     }
     // 8. exit (C29): level-n cell within arrive_cells of an exit cell
     if (role == 0 || fsm == 0) {
@@ -385,7 +422,7 @@ __device__ __forceinline__ void ped_step_one(const PedArgs<T> &a, const int d)
 // critical path of small crowds).  The chain fills N_p buffer parity ^ 1, which the flood kernel
 // running beside this one does not read.
 template <typename T>
-__global__ void __launch_bounds__(128) ped_step_kernel(PedArgs<T> a, int fuse_count)
+__global__ void __launch_bounds__(PED_THREADS) ped_step_kernel(PedArgs<T> a, int fuse_count)
 {
     pdl_enter();
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
