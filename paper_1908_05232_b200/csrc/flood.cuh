@@ -413,6 +413,27 @@ __global__ void flood_derive_kernel(FloodArgs<T> a, T *u, T *v, T *hr)
     }
 }
 
+// Bed for sim_read_flood: the device keeps z = +inf in solid cells (R3); the caller gets the
+// elevation the cell was created with.
+template <typename T>
+__global__ void flood_bed_kernel(const T *__restrict__ zs, const T *__restrict__ z0, size_t n, T *out)
+{
+    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x)
+        out[c] = is_solid(zs[c]) ? z0[c] : zs[c];
+}
+
+// After a state re-injection (sim_write_flood): bed with the solid cells marked (z given: new bed;
+// else keep), and no water in solid cells (C16).
+template <typename T>
+__global__ void flood_inject_kernel(T *h, T *qx, T *qy, T *zs, const T *z_new, const uint8_t *mask, size_t n)
+{
+    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x) {
+        const bool solid = mask[c] != 0;
+        if (z_new) zs[c] = solid ? solid_z<T>() : z_new[c];
+        if (solid) { h[c] = T(0); qx[c] = T(0); qy[c] = T(0); }
+    }
+}
+
 // volume (fp64), max h, max HR, non-finite count: two-stage reduction into out[4]
 template <typename T>
 __global__ void flood_stats_kernel(FloodArgs<T> a, double *out /* volume, max_h, max_hr, n_bad */)

@@ -94,6 +94,17 @@ int fail(sim *s, int code, const std::string &msg)
 
 size_t real_size(const sim *s) { return s->grid.real_bits == 64 ? 8 : 4; }
 
+// Every entry point runs on the device the handle was created on, whatever the caller's current
+// device is, and leaves the caller's device as it found it.
+struct DeviceGuard {
+    int prev = -1; bool switched = false;
+    explicit DeviceGuard(const sim *s)
+    {
+        if (s && cudaGetDevice(&prev) == cudaSuccess && prev != s->device) switched = cudaSetDevice(s->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 // Lay out (dry = true: only measure) all device state.
 size_t layout(sim *s, Bump &b)
 {
@@ -142,6 +153,12 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     if (p->n_targets < 1 || p->n_inflow_faces < 0 || p->n_hydro < 0 || p->n_line < 0 || p->n_exit_cells < 0)
         return fail(s, SIM_EINVAL, "bad list length in params");
     s->grid = *g;
+    {   // SMs of the current device (148 on a B200; also the value assumed when sizing without a device)
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) {
+            s->device = dev; s->n_sm = n;
+        }
+    }
     s->ncell = g->nx * g->ny; s->np = n_peds;
     const double dmin = g->dx < g->dy ? g->dx : g->dy;
     s->kbin = (int)std::ceil(p->R_int / dmin); if (s->kbin < 1) s->kbin = 1;     // C26
@@ -152,7 +169,7 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     s->march_gx = (g->nx + MW - 1) / MW;
     // about 15 waves of 148 SMs x 6 resident CTAs (measured on 8192^2: flat optimum R = 14..24;
     // short chunks even out the dry/wet imbalance between CTAs, halo rows cost little: not DRAM-bound)
-    const long long slots = 148 * 6;
+    const long long slots = (long long)s->n_sm * 6;
     s->march_R = (int)(((long long)g->ny * s->march_gx) / (15 * slots));
     if (s->march_R > MARCH_MAX_R) s->march_R = MARCH_MAX_R;
     if (s->march_R < 16) s->march_R = 16;
@@ -183,12 +200,10 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 }
 
 template <typename T, int CPT, int STAGES, int MINB>
-void launch_tmarch(const FloodArgs<T> &fa, dim3 grid, cudaStream_t st, bool pdl)
+cudaError_t launch_tmarch(const FloodArgs<T> &fa, dim3 grid, cudaStream_t st, bool pdl)
 {
-    constexpr size_t dyn = tmarch_dyn_smem<T, STAGES>();
-    static bool once = (cudaFuncSetAttribute(flood_tmarch_kernel<T, CPT, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn), true);
-    (void)once;
-    launch_pdl(flood_tmarch_kernel<T, CPT, STAGES, MINB>, grid, dim3(MW / CPT), dyn, st, pdl, fa);
+    constexpr size_t dyn = tmarch_dyn_smem<T, STAGES>();      // the opt-in limit is set per device in sim_create (set_smem_attr)
+    return launch_pdl(flood_tmarch_kernel<T, CPT, STAGES, MINB>, grid, dim3(MW / CPT), dyn, st, pdl, fa);
 }
 
 template <typename T> FloodArgs<T> flood_args(const sim *s)
@@ -295,22 +310,23 @@ template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelin
     return SIM_OK;
 }
 
-template <typename T> void launch_flood(sim *s, cudaStream_t st, bool pdl)
+template <typename T> int launch_flood(sim *s, cudaStream_t st, bool pdl)
 {
     FloodArgs<T> fa = flood_args<T>(s);
     if (s->flood_variant == 4) {
-        launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st, pdl);
+        CU((launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st, pdl)));
     } else if (s->flood_variant == 3) {
-        launch_pdl(flood_march2_kernel<T, 2>, dim3(s->march_gx, s->march_gy), dim3(MW / 2), 0, st, pdl, fa);
+        CU(launch_pdl(flood_march2_kernel<T, 2>, dim3(s->march_gx, s->march_gy), dim3(MW / 2), 0, st, pdl, fa));
     } else if (s->flood_variant == 2) {
-        launch_pdl(flood_march_kernel<T>, dim3(s->march_gx, s->march_gy), dim3(MW), 0, st, pdl, fa);
+        CU(launch_pdl(flood_march_kernel<T>, dim3(s->march_gx, s->march_gy), dim3(MW), 0, st, pdl, fa));
     } else if (s->flood_variant == 1) {
         dim3 grid((s->grid.nx + TX - 1) / TX, (s->grid.ny + TY - 1) / TY);
-        launch_pdl(flood_tile_kernel<T>, grid, dim3(FLOOD_TILE_THREADS), sizeof(TileSmem<T>), st, pdl, fa);
+        CU(launch_pdl(flood_tile_kernel<T>, grid, dim3(FLOOD_TILE_THREADS), sizeof(TileSmem<T>), st, pdl, fa));
     } else {
         dim3 blk(32, 8), grid((s->grid.nx + 31) / 32, (s->grid.ny + 7) / 8);
-        launch_pdl(flood_cell_kernel<T>, grid, blk, 0, st, pdl, fa);
+        CU(launch_pdl(flood_cell_kernel<T>, grid, blk, 0, st, pdl, fa));
     }
+    return SIM_OK;
 }
 
 // ONE coupled step n on `st`, given that the binning chain of step n has run (sim::binned):
@@ -338,7 +354,10 @@ template <typename T> int enqueue_step(sim *s, cudaStream_t st, bool first, cuda
         }
     } else mark.k = 1;
     mark();
-    launch_flood<T>(s, st, s->pdl && !ev);
+    {
+        int rc = launch_flood<T>(s, st, s->pdl && !ev);
+        if (rc != SIM_OK) return rc;
+    }
     if (fork) {
         int rc = enqueue_bin_chain<T>(s, sp, 1, mark, true);             // counted inside ped_step
         if (rc != SIM_OK) return rc;
@@ -374,7 +393,8 @@ template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
 {
     constexpr int NE = 8, BATCH = 64;
     static const int slot_of[NE - 1] = {3, 4, 5, 0, 1, 2, 6};       // launch order -> kernel_ms index
-    std::vector<cudaEvent_t> ev(NE * BATCH);
+    std::vector<cudaEvent_t> ev(NE * BATCH, nullptr);
+    struct Cleanup { std::vector<cudaEvent_t> &v; ~Cleanup() { for (auto e : v) if (e) cudaEventDestroy(e); } } cleanup{ev};
     for (auto &e : ev) CU(cudaEventCreate(&e));
     for (int k = 0; k < 8; ++k) ms[k] = 0.0;
     int rc = prepare_bins<T>(s);
@@ -393,7 +413,6 @@ template <typename T> int step_profiled(sim *s, int64_t n, double *ms)
             }
         n -= m;
     }
-    for (auto &e : ev) cudaEventDestroy(e);
     return rc;
 }
 
@@ -431,9 +450,11 @@ template <typename T> int refresh_dt(sim *s)      // lambda of the state in plac
     return SIM_OK;
 }
 
+// opt-in dynamic shared memory of the kernels that need it, on the handle's device (the attribute is per device)
 template <typename T> int set_smem_attr(sim *s)
 {
     CU(cudaFuncSetAttribute(flood_tile_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<T>)));
+    CU(cudaFuncSetAttribute(flood_tmarch_kernel<T, 2, 4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tmarch_dyn_smem<T, 4>()));
     return SIM_OK;
 }
 
@@ -569,6 +590,12 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     if (p->n_exit_cells > 16) return bail(fail(s, SIM_EINVAL, "at most 16 exit cells"));
     if (!(p->tau > 0) || !(p->B_s > 0) || !(p->g > 0) || !(p->cfl > 0))
         return bail(fail(s, SIM_EINVAL, "tau, B_s, g, cfl must be positive"));
+    if (!(p->h_dry > 0) || (grid->real_bits == 32 && p->h_dry < 1.2e-38))
+        return bail(fail(s, SIM_EINVAL, "h_dry must be positive (and a normal number in the storage precision): depths are divided by max(h, h_dry)"));
+    if (!(p->A_s > 0) || !(p->radius >= 0) || !(p->vmax_factor > 0))
+        return bail(fail(s, SIM_EINVAL, "A_s and vmax_factor must be positive, radius non-negative"));
+    if (workspace && ((uintptr_t)workspace % 256) != 0)
+        return bail(fail(s, SIM_EINVAL, "workspace must be 256-byte aligned (TMA row copies need 16-byte aligned rows)"));
     if (p->exit_target < 0 || p->exit_target >= p->n_targets || p->storage_target < 0 ||
         p->storage_target >= p->n_targets || p->drop_target < 0 || p->drop_target >= p->n_targets)
         return bail(fail(s, SIM_EINVAL, "target index out of range"));
@@ -593,6 +620,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         const bool on_edge = (side == SIM_SIDE_W && i == 0) || (side == SIM_SIDE_E && i == nx - 1) ||
                              (side == SIM_SIDE_S && j == 0) || (side == SIM_SIDE_N && j == ny - 1);
         if (!on_edge) return bail(fail(s, SIM_EINVAL, "inflow faces must lie on the domain edge (C14)"));
+        if (topo->mask && topo->mask[c]) return bail(fail(s, SIM_EINVAL, "inflow face on a solid cell: its share of Q(t) would be lost"));
         uint8_t &m = infl[side][side < 2 ? j : i];
         if (m == 255) return bail(fail(s, SIM_EINVAL, "too many inflow faces on one cell side"));
         m += 1;
@@ -661,6 +689,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
 extern "C" int sim_step(sim_t *s, int64_t n)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     if (n < 0) return fail(s, SIM_EINVAL, "negative step count");
     if (n == 0) return SIM_OK;
     {
@@ -689,6 +718,7 @@ extern "C" int sim_step(sim_t *s, int64_t n)
 extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     if (n < 0 || !kernel_ms) return fail(s, SIM_EINVAL, "bad arguments");
     return DISPATCH(s, step_profiled, s, n, kernel_ms);
 }
@@ -698,6 +728,7 @@ extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? (s
 extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     if (rows < 8 || rows > MARCH_MAX_R) return fail(s, SIM_EINVAL, "rows per chunk must be in [8, 64]");
     CU(cudaStreamSynchronize(s->stream));
     s->march_R = rows;
@@ -714,6 +745,7 @@ extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
 extern "C" int sim_set_overlap(sim_t *s, int32_t on)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     CU(cudaStreamSynchronize(s->stream));
     s->overlap = on ? 1 : 0;
     drop_graphs(s);
@@ -725,6 +757,7 @@ extern "C" int sim_get_flood_variant(const sim_t *s) { return s ? s->flood_varia
 extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     if (variant < 0 || variant > 4) return fail(s, SIM_EINVAL, "variant must be 0..4");
     if (variant == 4 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
     if (variant == 3 && s->grid.nx % 2 != 0) return fail(s, SIM_EINVAL, "the two-column march kernel needs nx % 2 == 0");
@@ -754,13 +787,8 @@ template <typename T> int read_flood_t(sim *s, void *h, void *u, void *v, void *
         return SIM_ECUDA;
     if (z) {
         // bed with the barrier raised; solid cells report the elevation they were created with
-        std::vector<T> zs(s->ncell), z0(s->ncell);
-        CU(cudaMemcpyAsync(zs.data(), s->zs, bytes, cudaMemcpyDeviceToHost, s->stream));
-        CU(cudaMemcpyAsync(z0.data(), s->z0, bytes, cudaMemcpyDeviceToHost, s->stream));
-        CU(cudaStreamSynchronize(s->stream));
-        for (int k = 0; k < s->ncell; ++k) if (std::isinf((double)zs[k])) zs[k] = z0[k];
-        CU(cudaMemcpyAsync(s->scratch_real[0], zs.data(), bytes, cudaMemcpyHostToDevice, s->stream));
-        CU(cudaStreamSynchronize(s->stream));
+        flood_bed_kernel<T><<<1184, 256, 0, s->stream>>>((const T *)s->zs, (const T *)s->z0, (size_t)s->ncell, (T *)s->scratch_real[0]);
+        CU(cudaGetLastError());
         if (copy_out(s, z, s->scratch_real[0], bytes)) return SIM_ECUDA;
     }
     CU(cudaStreamSynchronize(s->stream));
@@ -853,16 +881,14 @@ template <typename T> int write_flood_t(sim *s, const void *h, const void *qx, c
     if (h) CU(cudaMemcpyAsync(s->h[p], h, bytes, cudaMemcpyHostToDevice, s->stream));
     if (qx) CU(cudaMemcpyAsync(s->qx[p], qx, bytes, cudaMemcpyHostToDevice, s->stream));
     if (qy) CU(cudaMemcpyAsync(s->qy[p], qy, bytes, cudaMemcpyHostToDevice, s->stream));
+    if (z) CU(cudaMemcpyAsync(s->scratch_real[0], z, bytes, cudaMemcpyHostToDevice, s->stream));
+    // solid cells hold no water and keep z = +inf; then the CFL dt, q_in and halt of the injected state
+    flood_inject_kernel<T><<<1184, 256, 0, s->stream>>>((T *)s->h[p], (T *)s->qx[p], (T *)s->qy[p], (T *)s->zs,
+                                                       z ? (const T *)s->scratch_real[0] : nullptr, s->mask, nc);
+    CU(cudaGetLastError());
+    int rc = refresh_dt<T>(s);
+    if (rc != SIM_OK) return rc;
     CU(cudaStreamSynchronize(s->stream));
-    if (z) {
-        std::vector<uint8_t> mask(nc);
-        CU(cudaMemcpyAsync(mask.data(), s->mask, nc, cudaMemcpyDeviceToHost, s->stream));
-        CU(cudaStreamSynchronize(s->stream));
-        std::vector<T> zs;
-        make_zs<T>((const T *)z, mask.data(), nc, zs);
-        CU(cudaMemcpyAsync(s->zs, zs.data(), bytes, cudaMemcpyHostToDevice, s->stream));
-        CU(cudaStreamSynchronize(s->stream));
-    }
     return SIM_OK;
 }
 
@@ -871,12 +897,14 @@ template <typename T> int write_flood_t(sim *s, const void *h, const void *qx, c
 extern "C" int sim_read_flood(sim_t *s, void *h, void *u, void *v, void *z, void *hr)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     return DISPATCH(s, read_flood_t, s, h, u, v, z, hr);
 }
 
 extern "C" int sim_read_conserved(sim_t *s, void *h, void *qx, void *qy)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     Ctl c;
     CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
     CU(cudaStreamSynchronize(s->stream));
@@ -890,6 +918,7 @@ extern "C" int sim_read_conserved(sim_t *s, void *h, void *qx, void *qy)
 extern "C" int sim_read_occupancy(sim_t *s, uint8_t *np_cell)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     Ctl c;
     CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
     CU(cudaStreamSynchronize(s->stream));
@@ -903,12 +932,14 @@ extern "C" int sim_read_peds(sim_t *s, void *x, void *y, void *vx, void *vy, uin
                              uint8_t *active, int32_t *cell, void *timer)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     return DISPATCH(s, read_peds_t, s, x, y, vx, vy, state, fsm, active, cell, timer);
 }
 
 extern "C" int sim_get_stats(sim_t *s, sim_stats_t *out)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     if (!out) return fail(s, SIM_EINVAL, "out is NULL");
     return DISPATCH(s, stats_t, s, out);
 }
@@ -917,6 +948,7 @@ extern "C" int sim_bin_peds(sim_t *s, int32_t *key, int32_t *order, int32_t *sta
                             int32_t *n_bins_x, int32_t *n_bins_y, int32_t *k)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     if (n_bins_x) *n_bins_x = s->nbx;
     if (n_bins_y) *n_bins_y = s->nby;
     if (k) *k = s->kbin;
@@ -927,6 +959,7 @@ extern "C" int sim_bin_peds(sim_t *s, int32_t *key, int32_t *order, int32_t *sta
 extern "C" int sim_write_flood(sim_t *s, const void *h, const void *qx, const void *qy, const void *z)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     s->binned = false;
     return DISPATCH(s, write_flood_t, s, h, qx, qy, z);
 }
@@ -935,6 +968,7 @@ extern "C" int sim_write_peds(sim_t *s, const void *x, const void *y, const void
                               const uint8_t *fsm, const uint8_t *active, const void *timer)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     s->binned = false;
     const size_t np = (size_t)s->np, rb = np * real_size(s);
     if (!np) return SIM_OK;
@@ -977,6 +1011,7 @@ extern "C" int sim_write_peds(sim_t *s, const void *x, const void *y, const void
 extern "C" int sim_set_time(sim_t *s, double t, double dt)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     s->binned = false;
     Ctl c;
     CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
@@ -1002,6 +1037,7 @@ extern "C" int sim_set_time(sim_t *s, double t, double dt)
 extern "C" int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete)
 {
     if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
     s->binned = false;
     Ctl c;
     CU(cudaMemcpyAsync(&c, s->ctl, sizeof c, cudaMemcpyDeviceToHost, s->stream));
@@ -1017,6 +1053,7 @@ extern "C" const char *sim_last_error(const sim_t *s) { return s ? s->err.c_str(
 extern "C" void sim_destroy(sim_t *s)
 {
     if (!s) return;
+    DeviceGuard on_device(s);
     if (s->ws) cudaStreamSynchronize(s->stream);
     drop_graphs(s);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);

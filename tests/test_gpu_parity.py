@@ -290,9 +290,39 @@ def test_config2_multi_step_aggregates_fp32():
     assert abs(a["t"] - b["t"]) <= 1e-4 * b["t"]
     assert abs(a["volume"] - b["volume"]) <= 1e-4 * b["volume"]      # fp32 storage of h: 1e-5 per DESIGN + dt drift
     assert abs(a["max_h"] - b["max_h"]) <= 1e-3 * b["max_h"]
-    # chaotic fp32 crowd at the exit queue (order inside a bin, hence the summation order, is not
-    # fixed): at most 1 % of the agents may sit in another class; each of them counts twice in L1
-    assert sum(abs(x - y) for x, y in zip(a["hist"], b["hist"])) <= 0.02 * sc.n_peds
+    # histogram: at most 1 % of the agents in another class than the oracle's, i.e. an L1
+    # distance <= 2 % of the agents (an agent in another class is counted in two classes).  This run is
+    # the one calibrated case that needs it: a thin wetting film (h near h_dry = 1 mm) spreads under a
+    # crowd queueing at the exit, so dry/low flips with the last bits of h and of the chaotic fp32
+    # positions (measured: L1 = 32 of 2000 = 16 agents).  Config 1 (fp64) and Config 4 are exact.
+    l1 = sum(abs(x - y) for x, y in zip(a["hist"], b["hist"]))
+    print(f"config2 x10 inflow, 600 steps: hist L1 = {l1} of {sc.n_peds} agents, volume rel {abs(a['volume'] - b['volume']) / b['volume']:.2e}")
+    assert l1 <= 0.02 * sc.n_peds
+
+
+def test_config4_multi_step_aggregates_fp32():
+    """Config 4 recipe (multi-octave bed, Manning n per cell, 25 % building blocks, reservoir dam
+    break, 100 000 pedestrians at full size) at a size the oracle follows in under a minute:
+    1024^2 cells, 25 000 pedestrians, 200 coupled steps, compared on the aggregates of DESIGN.md 5.4.
+    The full 2048^2 x 1000-step run against the oracle is quoted in BASELINE.md."""
+    sc = S.make(4, n=1024, n_peds=25_000)
+    o = oracle.Oracle(sc); g = binding.Sim(sc)
+    o.step(200); g.step(200)
+    a, b = g.stats(), o.stats()
+    assert a["step"] == b["step"] == 200
+    l1 = sum(abs(x - y) for x, y in zip(a["hist"], b["hist"]))
+    c, d = g.read_conserved(), o.read_conserved()
+    l1_field = float(np.abs(c["h"].astype(np.float64) - d["h"]).sum() / np.abs(d["h"]).sum())
+    print(f"config4 at 1024^2, 200 steps: t {a['t']:.5f} / {b['t']:.5f}, volume rel {abs(a['volume'] - b['volume']) / b['volume']:.2e}, "
+          f"max_h rel {abs(a['max_h'] - b['max_h']) / b['max_h']:.2e}, hist L1 {l1}, clamps {a['neg_depth_clamps']} / {b['neg_depth_clamps']}, "
+          f"depth field L1 rel {l1_field:.2e}, max-norm {mixed(c['h'], d['h']):.2e}")
+    assert abs(a["t"] - b["t"]) <= 1e-4 * b["t"]
+    assert abs(a["volume"] - b["volume"]) <= 1e-4 * b["volume"]
+    assert abs(a["max_h"] - b["max_h"]) <= 1e-3 * b["max_h"]
+    assert l1 <= 0.01 * sc.n_peds
+    # the depth field itself after 200 fp32 steps: in L1 (a cell at a steep dam-break front may differ by
+    # 1e-3 of the maximum depth after 200 steps of fp32 rounding; the field as a whole does not)
+    assert l1_field <= 1e-5
 
 
 def test_t_end_lands_and_halts_on_device():
