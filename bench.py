@@ -33,9 +33,21 @@ import numpy as np  # noqa: E402
 
 FLOOD_BYTES_PER_CELL = 33        # fp32: read h,qx,qy,z,n0 (20) + N_p (1) ; write h,qx,qy (12)  [DESIGN.md 6]
 PED_BYTES_PER_AGENT = 175        # key+count 17, scatter 72, step 85
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the flood kernel, from the committed
-# ncu --set full capture (profiles/r1_final_ncu_full_c5.md); only for the exact workload profiled
-NCU_TRAFFIC_BYTES = {(5, 4): 1.588444e9 + 770.069e6}
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
+
+
+def ncu_traffic(cfg, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on config `cfg`, as recorded by
+    the last committed `ncu --set full` capture (written by paper_1908_05232_b200/ncu_summary.py; a
+    profiler cannot run inside a timed bench, so this is a STATIC record of that capture, or None)."""
+    try:
+        rec = json.load(open(TRAFFIC_JSON)).get(f"config{cfg}", {})
+    except (OSError, ValueError):
+        return None, None
+    for name, r in rec.items():
+        if kernel in name:
+            return r["dram_bytes_read"] + r["dram_bytes_write"], f"static: ncu capture summarised in profiles/{r['summary']}"
+    return None, None
 
 
 def peaks():
@@ -91,19 +103,22 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def scenario(cfg, small=False):
+def scenario(cfg):
     from paper_1908_05232_b200 import scenarios as S
-    if small:                       # CPU-oracle sample: same recipe, bounded size
-        kw = {1: {}, 2: {}, 3: {}, 4: dict(n=1024, n_peds=25_000), 5: dict(n=2048, n_peds=62_500)}[cfg]
-    else:
-        kw = {}
-    return S.make(cfg, **kw)
+    return S.make(cfg)
 
 
-def oracle_run(cfg, steps, warmup):
-    """The oracle as it stands, single thread, on the bounded sample; returns (cells/s, agents/s, s/step, desc)."""
+# coupled steps of the CPU oracle that make a bounded sample of each config (Config 5 is
+# timed over 5 steps after 1 warm-up; about 10 s per step and 8 GB at 8192^2 cells + 1e6 pedestrians)
+ORACLE_STEPS = {1: 1000, 2: 2000, 3: 2000, 4: 20, 5: 5}
+
+
+def oracle_run(cfg, steps, warmup, sc=None):
+    """The oracle as it stands, single thread, on the SAME workload (full size), over a bounded
+    number of coupled steps; returns (cells/s, agents/s, s/step, desc)."""
     import oracle
-    sc = scenario(cfg, small=True)
+    if sc is None:
+        sc = scenario(cfg)
     o = oracle.Oracle(sc)
     if warmup:
         o.step(warmup)
@@ -120,15 +135,17 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    steps = min(args.steps, {1: 1000, 2: 2000, 3: 2000, 4: 24, 5: 20}[args.config])
+    steps = min(args.steps, ORACLE_STEPS[args.config])
     warm = min(args.warmup, 1)
     cps, aps, sps, desc = oracle_run(args.config, steps, warm)
+    done_steps = steps
     line = {
         "impl": "reference", "metric": "flood cell-updates/s (coupled step)", "value": cps, "unit": "cell-updates/s",
         "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * sps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "agent_updates_per_s": aps, "coupled_steps_per_s": 1.0 / sps,
         "config": {"workload": f"config{args.config}", "sample": desc},
+        "timed_steps": done_steps,
         "cpu_baseline": {"value": cps, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": desc},
         "e2e": {"value": cps, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -220,12 +237,24 @@ def run_ours(args):
         pad = np.pad(cnt, 1)
         nb9 = sum(pad[dj:dj + b["nby"], di:di + b["nbx"]] for dj in range(3) for di in range(3))
         cand = float((cnt * nb9).sum())
+        # the method's own work: ordered pairs with 0 < d < R_int (C26), counted with a k-d tree
+        from scipy.spatial import cKDTree
+        pp = g.read_peds()
+        live = pp["active"] == 1
+        tree = cKDTree(np.c_[pp["x"][live].astype(np.float64), pp["y"][live].astype(np.float64)])
+        inter = float(tree.count_neighbors(tree, sc.R_int)) - float(live.sum())
         ped_step_ms = kms["ped_step"] / KP
         xu_peak = 148 * 16 * 1.965e9 / 1e12          # 16 MUFU lanes per SM and clock (4 per SMSP), 148 SMs, 1965 MHz
-        xu = {"bound": "alu", "pipe": "xu (MUFU)", "kernel": "ped_step_kernel", "achieved": 2.0 * cand / (ped_step_ms * 1e-3) / 1e12,
-              "peak": xu_peak, "unit": "T MUFU/s", "frac": 2.0 * cand / (ped_step_ms * 1e-3) / 1e12 / xu_peak,
-              "candidate_pairs_per_step": cand, "candidates_per_agent": cand / max(active, 1), "ms": ped_step_ms,
-              "peak_source": "derived: 148 SMs x 16 MUFU/clk x 1.965 GHz (DESIGN.md 7); ncu XU pipe 70.6 % (profiles/r1_final_ncu_full_c5.md)"}
+        xu = {"bound": "alu", "pipe": "xu (MUFU)", "kernel": "ped_step_kernel",
+              "achieved": 2.0 * inter / (ped_step_ms * 1e-3) / 1e12, "peak": xu_peak, "unit": "T MUFU/s",
+              "frac": 2.0 * inter / (ped_step_ms * 1e-3) / 1e12 / xu_peak,
+              "work": "2 MUFU (rsqrt, ex2) per INTERACTING ordered pair (d < R_int): the method's own work",
+              "interacting_pairs_per_step": inter, "interacting_per_agent": inter / max(active, 1),
+              "candidate_pairs_per_step": cand, "candidates_per_agent": cand / max(active, 1),
+              "issued": {"achieved": 2.0 * cand / (ped_step_ms * 1e-3) / 1e12, "frac": 2.0 * cand / (ped_step_ms * 1e-3) / 1e12 / xu_peak,
+                         "note": "MUFU operations the kernel ISSUES: 2 per candidate of the 3 x 3 bins (a predicated-off MUFU still occupies the pipe for the warp)"},
+              "ms": ped_step_ms,
+              "peak_source": "derived: 148 SMs x 16 MUFU/clk x 1.965 GHz (DESIGN.md 7)"}
 
     # ---- end to end through the C ABI with pinned HOST buffers
     host = {k: torch.empty(ncell, dtype=torch.float32 if real is np.float32 else torch.float64).pin_memory()
@@ -260,14 +289,16 @@ def run_ours(args):
         return
 
     # ---- CPU oracle, bounded sample (reported baseline, not the target)
-    o_steps = {1: 1000, 2: 2000, 3: 2000, 4: 24, 5: 20}[args.config]     # about 10 s of one host core
+    o_steps = ORACLE_STEPS[args.config]
     if world == 1 and not args.no_cpu_baseline:
-        cps, aps, sps, desc = oracle_run(args.config, o_steps, 1)
+        cps, aps, sps, desc = oracle_run(args.config, o_steps, 1, sc)
         cpu = {"value": cps, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": desc,
                "agent_updates_per_s": aps}
     else:
         cpu = None
 
+    kernel_name = ("flood_cell_kernel", "flood_tile_kernel", "flood_march_kernel", "flood_march2_kernel", "flood_tmarch_kernel")[variant]
+    traffic, traffic_src = ncu_traffic(args.config, kernel_name) if args.march_rows == 0 and args.flood_variant < 0 else (None, None)
     agg = aggregate(ms_max, world, ncell, done, active)
     line = {
         "metric": "flood cell-updates/s (coupled step)", "value": agg["value"], "unit": "cell-updates/s",
@@ -287,12 +318,12 @@ def run_ours(args):
                 "steps": e2e_done, "seconds": e2e_s,
                 "what": "sim_write_flood+sim_write_peds from pinned host, sim_step, sim_read_conserved+sim_read_peds+sim_get_stats to host"},
         "gpu_launches": int(done * kps),
-        "roofline": {"bound": "hbm", "kernel": ("flood_cell_kernel", "flood_tile_kernel", "flood_march_kernel", "flood_march2_kernel", "flood_tmarch_kernel")[variant] + ("<float>" if sc.real_bits == 32 else "<double>"),
+        "roofline": {"bound": "hbm", "kernel": kernel_name + ("<float>" if sc.real_bits == 32 else "<double>"),
                      "achieved": flood_gbs, "peak": peak, "unit": "GB/s", "frac": flood_gbs / peak,
                      "peak_source": peak_src, "frac_of_8TBs_spec": flood_gbs / 8000.0,
                      "bytes_per_cell": fb, "kernel_ms": flood_ms,
-                     "traffic": NCU_TRAFFIC_BYTES.get((args.config, variant)) if args.march_rows == 0 else None,
-                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_final_ncu_full_c5.md)",
+                     "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+                     "traffic_source": traffic_src,
                      "algorithmic_bytes": ncell * fb,
                      "timed_with": f"cudaEvent before each launch over {KP} steps (sim_step_profiled) right after the timed region"},
         "kernels_ms_per_step": {k: v / KP for k, v in kms.items()},
