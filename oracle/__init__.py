@@ -44,6 +44,7 @@ class OrcConfig(C.Structure):
         ("bags_per_cell_layer", C.c_int), ("n_layers", C.c_int),
         ("layer_thickness", C.c_double), ("t_pick", C.c_double), ("t_drop", C.c_double),
         ("t_end", C.c_double),
+        ("flood_order", C.c_int),
     ]
 
 
@@ -80,6 +81,8 @@ def lib():
         L.orc_riemann_flux.restype = None
         L.orc_face.argtypes = [d] * 9 + [_dp, _dp, _dp]
         L.orc_face.restype = None
+        L.orc_minmod.argtypes = [d, d]
+        L.orc_minmod.restype = d
         L.orc_friction.argtypes = [d, d, d, d, d, _dp, _dp]
         L.orc_friction.restype = None
         L.orc_cell_dt.argtypes = [d] * 7
@@ -147,6 +150,10 @@ def face(g, hi, uni, uti, zi, hk, unk, utk, zk):
     fi, fk = C.c_double(), C.c_double()
     lib().orc_face(g, hi, uni, uti, zi, hk, unk, utk, zk, out, C.byref(fi), C.byref(fk))
     return np.array(out[:]), fi.value, fk.value
+
+
+def minmod(a, b):
+    return lib().orc_minmod(a, b)
 
 
 def friction(g, n, dt, h_dry, h, qx, qy):
@@ -246,6 +253,7 @@ class Oracle:
         cfg.bags_per_cell_layer, cfg.n_layers = sc.bags_per_cell_layer, sc.n_layers
         cfg.layer_thickness, cfg.t_pick, cfg.t_drop = sc.layer_thickness, sc.t_pick, sc.t_drop
         cfg.t_end = sc.t_end
+        cfg.flood_order = int(getattr(sc, "flood_order", 1))
         self._h = L.orc_create(C.byref(cfg))
         if not self._h:
             raise ValueError("orc_create failed")

@@ -27,6 +27,7 @@ struct orc_sim {
     orc_config c;                 /* scalar copy; pointers below are owned copies */
     int ncell;
     double *z, *n0, *h, *qx, *qy, *h1, *qx1, *qy1;
+    double *fv[4][4];             /* second-order variant: predicted (h, qx, qy, z) at the W, E, S, N face of every cell */
     unsigned char *mask;
     int *Np;
     int *inflow_mult[4];          /* per side, how many listed inflow faces sit on that cell side */
@@ -274,6 +275,8 @@ orc_sim *orc_create(const orc_config *cfg)
         s->qx[c] = s->h[c] * (cfg->u0 ? cfg->u0[c] : 0.0);   /* store conserved (S:8c-C8) */
         s->qy[c] = s->h[c] * (cfg->v0 ? cfg->v0[c] : 0.0);
     }
+    if (cfg->flood_order == 2)
+        for (int f = 0; f < 4; ++f) for (int k = 0; k < 4; ++k) s->fv[f][k] = dup_mem(NULL, nb);
     s->Np = dup_mem(NULL, (size_t)nc * sizeof(int));
     s->inflow_length = 0.0;
     for (int k = 0; k < 4; ++k) s->inflow_mult[k] = dup_mem(NULL, (size_t)nc * sizeof(int));
@@ -343,6 +346,7 @@ void orc_destroy(orc_sim *s)
         s->timer1, s->role, s->state, s->fsm, s->active, s->state1, s->fsm1, s->active1, s->cell,
         s->head, s->next };
     for (size_t k = 0; k < sizeof p / sizeof p[0]; ++k) free(p[k]);
+    for (int f = 0; f < 4; ++f) for (int k = 0; k < 4; ++k) free(s->fv[f][k]);
     free(s);
 }
 
@@ -408,6 +412,147 @@ static void flood_step(orc_sim *s, double q_in)
             /* accounted clamp (S:8c-C12) */
             if (hn < 0.0) { s->clamped_volume += -hn * dx * dy; s->neg_clamps += 1; hn = 0.0; }
             /* Manning friction with the occupancy-dependent roughness */
+            double n = s->c.couple_roughness ? orc_roughness(s->n0[c], s->Np[c], s->c.n_cap) : s->n0[c];
+            orc_friction(g, n, dt, s->c.h_dry, hn, &qxn, &qyn);
+            s->h1[c] = hn; s->qx1[c] = qxn; s->qy1[c] = qyn;
+        }
+}
+
+/* ------------------------------------------------------------------ second order
+ * MUSCL-Hancock variant of the flood step: the second-order scheme the paper "reduced to
+ * first-order accuracy".  The paper prints none of it; this is the reading of
+ * DESIGN.md M1-M7, on top of the same face flux (orc_face), clamp and friction as flood_step():
+ *  M1 limited slopes of (eta, h, qx, qy), minmod, per direction; zero in a direction where the
+ *     cell or a neighbour is not wet (h <= h_dry) or a neighbour is a wall (edge, solid cell):
+ *     the scheme falls back to first order at wet/dry fronts and walls;
+ *  M2 face values W_i +- sigma/2; bed at a face z_f = eta_f - h_f;
+ *  M3 Hancock predictor: the four face values advance half a step with the physical fluxes of
+ *     the cell's own face values, pressure and bed slope together as g hbar (eta_E - eta_W)
+ *     (still water: no change), depth clamped at 0;
+ *  M4 one Riemann flux per face on the hydrostatically reconstructed predicted face states; the
+ *     momentum flux seen by a cell is F1 - g h*^2/2 + g h_f^2/2 with h_f its own face depth;
+ *  M5 centred bed-slope source g (h_W + h_E)(z_W - z_E) / 2 dx of the cell's own face values;
+ *  M6 update, inflow, clamp, friction as in the first-order step;  M7 same CFL rule.
+ * A cell whose slopes all vanish takes exactly the first-order step. */
+double orc_minmod(double a, double b)
+{
+    if (a * b <= 0.0) return 0.0;
+    return fabs(a) < fabs(b) ? a : b;
+}
+
+enum { FV_H = 0, FV_QX = 1, FV_QY = 2, FV_Z = 3 };
+
+static int is_wall(const orc_sim *s, int i, int j)
+{
+    if (i < 0 || j < 0 || i >= s->c.nx || j >= s->c.ny) return 1;
+    return s->mask[j * s->c.nx + i] != 0;
+}
+
+/* M1: limited slopes of (eta, h, qx, qy) of cell c along (di, dj) */
+static void muscl_slopes(const orc_sim *s, int i, int j, int di, int dj, double sl[4])
+{
+    sl[0] = sl[1] = sl[2] = sl[3] = 0.0;
+    if (is_wall(s, i - di, j - dj) || is_wall(s, i + di, j + dj)) return;
+    const int nx = s->c.nx, c = j * nx + i, a = (j - dj) * nx + (i - di), b = (j + dj) * nx + (i + di);
+    if (!(s->h[c] > s->c.h_dry && s->h[a] > s->c.h_dry && s->h[b] > s->c.h_dry)) return;
+    sl[0] = orc_minmod((s->h[c] + s->z[c]) - (s->h[a] + s->z[a]), (s->h[b] + s->z[b]) - (s->h[c] + s->z[c]));
+    sl[1] = orc_minmod(s->h[c] - s->h[a], s->h[b] - s->h[c]);
+    sl[2] = orc_minmod(s->qx[c] - s->qx[a], s->qx[b] - s->qx[c]);
+    sl[3] = orc_minmod(s->qy[c] - s->qy[a], s->qy[b] - s->qy[c]);
+}
+
+/* velocity of a face value of a WET cell: q / max(h, h_dry) (continuous in h); a cell that is not
+ * wet has u = v = 0 as in the first-order step */
+static double face_vel(const orc_sim *s, int cell_wet, double q, double h)
+{
+    return cell_wet ? q / fmax(h, s->c.h_dry) : 0.0;
+}
+
+static void muscl_predict(orc_sim *s)
+{
+    const double g = s->c.g, dt = s->dt, dx = s->c.dx, dy = s->c.dy;
+    const int nx = s->c.nx, ny = s->c.ny;
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            const int c = j * nx + i;
+            if (s->mask[c]) continue;
+            const double h = s->h[c], z = s->z[c], eta = h + z, qx = s->qx[c], qy = s->qy[c];
+            const int wet = h > s->c.h_dry;
+            double sx[4], sy[4];
+            muscl_slopes(s, i, j, 1, 0, sx);
+            muscl_slopes(s, i, j, 0, 1, sy);
+            /* M2: face values; index 0 W, 1 E, 2 S, 3 N */
+            double fe[4], fh[4], fqx[4], fqy[4], fz[4];
+            for (int f = 0; f < 4; ++f) {
+                const double *sl = f < 2 ? sx : sy;
+                const double sg = (f == ORC_E || f == ORC_N) ? 0.5 : -0.5;
+                fe[f] = eta + sg * sl[0]; fh[f] = h + sg * sl[1];
+                fqx[f] = qx + sg * sl[2]; fqy[f] = qy + sg * sl[3];
+                fz[f] = fe[f] - fh[f];
+            }
+            /* M3: Hancock predictor from the cell's own face values */
+            const double uE = face_vel(s, wet, fqx[ORC_E], fh[ORC_E]), uW = face_vel(s, wet, fqx[ORC_W], fh[ORC_W]);
+            const double vN = face_vel(s, wet, fqy[ORC_N], fh[ORC_N]), vS = face_vel(s, wet, fqy[ORC_S], fh[ORC_S]);
+            const double dh = -0.5 * dt / dx * (fqx[ORC_E] - fqx[ORC_W]) - 0.5 * dt / dy * (fqy[ORC_N] - fqy[ORC_S]);
+            const double dqx = -0.5 * dt / dx * ((fqx[ORC_E] * uE - fqx[ORC_W] * uW)
+                                                + g * 0.5 * (fh[ORC_E] + fh[ORC_W]) * (fe[ORC_E] - fe[ORC_W]))
+                               - 0.5 * dt / dy * (fqx[ORC_N] * vN - fqx[ORC_S] * vS);
+            const double dqy = -0.5 * dt / dx * (fqy[ORC_E] * uE - fqy[ORC_W] * uW)
+                               - 0.5 * dt / dy * ((fqy[ORC_N] * vN - fqy[ORC_S] * vS)
+                                                  + g * 0.5 * (fh[ORC_N] + fh[ORC_S]) * (fe[ORC_N] - fe[ORC_S]));
+            for (int f = 0; f < 4; ++f) {
+                s->fv[f][FV_H][c] = fmax(0.0, fh[f] + dh);
+                s->fv[f][FV_QX][c] = fqx[f] + dqx;
+                s->fv[f][FV_QY][c] = fqy[f] + dqy;
+                s->fv[f][FV_Z][c] = fz[f];
+            }
+        }
+}
+
+/* predicted state of cell c at its face f as (h, normal velocity, tangential velocity, z) */
+static void muscl_face_state(const orc_sim *s, int c, int f, double *h, double *un, double *ut, double *z)
+{
+    const int wet = s->h[c] > s->c.h_dry;
+    *h = s->fv[f][FV_H][c]; *z = s->fv[f][FV_Z][c];
+    const double u = face_vel(s, wet, s->fv[f][FV_QX][c], *h), v = face_vel(s, wet, s->fv[f][FV_QY][c], *h);
+    if (f < 2) { *un = u; *ut = v; } else { *un = v; *ut = u; }
+}
+
+static void flood_step_muscl(orc_sim *s, double q_in)
+{
+    const double g = s->c.g, dt = s->dt, dx = s->c.dx, dy = s->c.dy;
+    const int nx = s->c.nx, ny = s->c.ny;
+    muscl_predict(s);
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            const int c = j * nx + i;
+            if (s->mask[c]) { s->h1[c] = s->qx1[c] = s->qy1[c] = 0.0; continue; }
+            /* M4: the four faces; f = side of THIS cell, the neighbour contributes its opposite face */
+            double F0[4], Fn[4], Ft[4], hf[4], zf[4];
+            for (int f = 0; f < 4; ++f) {
+                const int di = (f == ORC_E) - (f == ORC_W), dj = (f == ORC_N) - (f == ORC_S);
+                double hi, uni, uti, zi, hk, unk, utk, zk, F[3], Fi, Fk;
+                muscl_face_state(s, c, f, &hi, &uni, &uti, &zi);
+                if (is_wall(s, i + di, j + dj)) { hk = hi; unk = -uni; utk = uti; zk = zi; }   /* wall ghost (S:8c-O2.1) */
+                else muscl_face_state(s, (j + dj) * nx + (i + di), f ^ 1, &hk, &unk, &utk, &zk);
+                if (f == ORC_E || f == ORC_N) { orc_face(g, hi, uni, uti, zi, hk, unk, utk, zk, F, &Fi, &Fk); }
+                else                          { orc_face(g, hk, unk, utk, zk, hi, uni, uti, zi, F, &Fk, &Fi); }
+                F0[f] = F[0]; Fn[f] = Fi + 0.5 * g * hi * hi; Ft[f] = F[2];
+                hf[f] = hi; zf[f] = zi;
+            }
+            /* inflow faces as in the first-order step (S:8c-O2.1, C14) */
+            F0[ORC_W] += q_in * s->inflow_mult[ORC_W][c];
+            F0[ORC_E] -= q_in * s->inflow_mult[ORC_E][c];
+            F0[ORC_S] += q_in * s->inflow_mult[ORC_S][c];
+            F0[ORC_N] -= q_in * s->inflow_mult[ORC_N][c];
+            /* M5: centred bed-slope source of the cell's own (predicted) face values */
+            const double Sx = 0.5 * g * (hf[ORC_W] + hf[ORC_E]) * (zf[ORC_W] - zf[ORC_E]) / dx;
+            const double Sy = 0.5 * g * (hf[ORC_S] + hf[ORC_N]) * (zf[ORC_S] - zf[ORC_N]) / dy;
+            /* M6: Eq. (2) with the second-order fluxes */
+            double hn  = s->h[c]  - dt / dx * (F0[ORC_E] - F0[ORC_W]) - dt / dy * (F0[ORC_N] - F0[ORC_S]);
+            double qxn = s->qx[c] - dt / dx * (Fn[ORC_E] - Fn[ORC_W]) - dt / dy * (Ft[ORC_N] - Ft[ORC_S]) + dt * Sx;
+            double qyn = s->qy[c] - dt / dx * (Ft[ORC_E] - Ft[ORC_W]) - dt / dy * (Fn[ORC_N] - Fn[ORC_S]) + dt * Sy;
+            if (hn < 0.0) { s->clamped_volume += -hn * dx * dy; s->neg_clamps += 1; hn = 0.0; }
             double n = s->c.couple_roughness ? orc_roughness(s->n0[c], s->Np[c], s->c.n_cap) : s->n0[c];
             orc_friction(g, n, dt, s->c.h_dry, hn, &qxn, &qyn);
             s->h1[c] = hn; s->qx1[c] = qxn; s->qy1[c] = qyn;
@@ -527,7 +672,7 @@ int orc_step(orc_sim *s, long long n)
         /* O2 */
         double Q = orc_hydrograph(s->c.n_hydro, s->hydro_t, s->hydro_q, s->t);
         double q_in = (s->inflow_length > 0.0) ? Q / s->inflow_length : 0.0;
-        flood_step(s, q_in);
+        if (s->c.flood_order == 2) flood_step_muscl(s, q_in); else flood_step(s, q_in);
         /* O3 (reads level-n flood and pedestrians) */
         long long D = ped_step(s);
         /* O4 */

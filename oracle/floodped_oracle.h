@@ -76,6 +76,9 @@ typedef struct {
     int bags_per_cell_layer, n_layers;
     double layer_thickness, t_pick, t_drop;
     double t_end;
+    /* ---- widened scope; zero-initialised = the paper's first-order closed-wall scheme ---- */
+    int flood_order;             /* 0 or 1: first order ("reduced to first-order accuracy");
+                                    2: MUSCL-Hancock, the second-order scheme it was reduced from (M1-M7) */
 } orc_config;
 
 typedef struct {
@@ -102,6 +105,8 @@ void orc_riemann_flux(double g, double hL, double unL, double utL,
 void orc_face(double g, double hi, double uni, double uti, double zi,
               double hk, double unk, double utk, double zk,
               double F[3], double *Fn_seen_by_i, double *Fn_seen_by_k);
+/* minmod slope limiter of the second-order variant (M1) */
+double orc_minmod(double a, double b);
 /* pointwise semi-implicit Manning friction, S:8c-O2.4 */
 void orc_friction(double g, double n, double dt, double h_dry, double h,
                   double *qx, double *qy);

@@ -85,6 +85,8 @@ class Scenario:
     t_drop: float = 30.0
     t_end: float = float("inf")
     steps: int = 0                           # the run length the config names (0: until t_end)
+    # widened scope
+    flood_order: int = 1                     # 1: the paper's first-order scheme; 2: MUSCL-Hancock (8f-2)
 
     @property
     def real(self):
