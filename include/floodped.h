@@ -120,6 +120,11 @@ typedef struct {
     int32_t        bags_per_cell_layer, n_layers;
     double  layer_thickness, t_pick, t_drop;    /* 0.25 m, 30 s, 30 s                     */
     double  t_end;                              /* steps are no-ops once t >= t_end; INFINITY = off */
+    /* accuracy of the flood step: 0 or 1 = the paper's scheme, "reduced to first-order accuracy"
+     * (P:L97); 2 = the second-order MUSCL-Hancock scheme it was reduced from (reading
+     * M1-M7 of DESIGN.md): minmod slopes, Hancock half-step predictor, same HLLC flux, hydrostatic
+     * reconstruction, friction and CFL rule */
+    int32_t flood_order;
 } sim_params_t;
 
 typedef struct {
@@ -181,7 +186,8 @@ int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32
  * face once, rows prefetched in registers (any nx); 3 = as 2 with two columns per thread and
  * 64/128-bit accesses (nx % 2 == 0); 4 = as 3 with the rows of interior chunks brought in by TMA
  * bulk copies into a shared-memory ring (nx % 16 == 0).
- * Default: from 2^22 cells 4 (else 3, else 2), below that 1 (or 0). */
+ * Default: from 2^22 cells 4 (else 3, else 2), below that 1 (or 0).  With flood_order = 2 the
+ * kernel is the MUSCL-Hancock tile kernel (reported as variant 5) and cannot be changed. */
 int sim_set_flood_variant(sim_t *s, int32_t variant);
 int sim_get_flood_variant(const sim_t *s);         /* the kernel in use, or SIM_EINVAL */
 /* Rows per chunk of the row-marching kernels (8..64; default chosen by sim_create). Tuning hook. */

@@ -60,6 +60,7 @@ class SimParams(C.Structure):
         ("bags_per_cell_layer", C.c_int32), ("n_layers", C.c_int32),
         ("layer_thickness", C.c_double), ("t_pick", C.c_double), ("t_drop", C.c_double),
         ("t_end", C.c_double),
+        ("flood_order", C.c_int32),
     ]
 
 
@@ -178,6 +179,7 @@ class _Marshalled:
         p.line_cells = typed(sc.line_cells, np.int32, _i32p)
         p.bags_per_cell_layer, p.n_layers = sc.bags_per_cell_layer, sc.n_layers
         p.layer_thickness, p.t_pick, p.t_drop, p.t_end = sc.layer_thickness, sc.t_pick, sc.t_drop, sc.t_end
+        p.flood_order = int(getattr(sc, "flood_order", 1))
         self.params = p
 
 

@@ -15,6 +15,7 @@
 #include "flood_march.cuh"
 #include "flood_march2.cuh"
 #include "flood_tmarch.cuh"
+#include "flood_muscl.cuh"
 #include "peds.cuh"
 
 using namespace fp;
@@ -313,7 +314,10 @@ template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelin
 template <typename T> int launch_flood(sim *s, cudaStream_t st, bool pdl)
 {
     FloodArgs<T> fa = flood_args<T>(s);
-    if (s->flood_variant == 4) {
+    if (s->flood_variant == 5) {                     // second order (flood_order = 2)
+        dim3 grid((s->grid.nx + MTX - 1) / MTX, (s->grid.ny + MTY - 1) / MTY);
+        CU(launch_pdl(flood_muscl_kernel<T>, grid, dim3(MTX, MTY), sizeof(MusclSmem<T>), st, pdl, fa));
+    } else if (s->flood_variant == 4) {
         CU((launch_tmarch<T, 2, 4, 6>(fa, dim3(s->march_gx, s->march_gy), st, pdl)));
     } else if (s->flood_variant == 3) {
         CU(launch_pdl(flood_march2_kernel<T, 2>, dim3(s->march_gx, s->march_gy), dim3(MW / 2), 0, st, pdl, fa));
@@ -455,6 +459,7 @@ template <typename T> int set_smem_attr(sim *s)
 {
     CU(cudaFuncSetAttribute(flood_tile_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<T>)));
     CU(cudaFuncSetAttribute(flood_tmarch_kernel<T, 2, 4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tmarch_dyn_smem<T, 4>()));
+    CU(cudaFuncSetAttribute(flood_muscl_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MusclSmem<T>)));
     return SIM_OK;
 }
 
@@ -592,6 +597,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         return bail(fail(s, SIM_EINVAL, "tau, B_s, g, cfl must be positive"));
     if (!(p->h_dry > 0) || (grid->real_bits == 32 && p->h_dry < 1.2e-38))
         return bail(fail(s, SIM_EINVAL, "h_dry must be positive (and a normal number in the storage precision): depths are divided by max(h, h_dry)"));
+    if (p->flood_order < 0 || p->flood_order > 2) return bail(fail(s, SIM_EINVAL, "flood_order must be 0, 1 (first order, the paper's scheme) or 2 (MUSCL-Hancock)"));
     if (!(p->A_s > 0) || !(p->radius >= 0) || !(p->vmax_factor > 0))
         return bail(fail(s, SIM_EINVAL, "A_s and vmax_factor must be positive, radius non-negative"));
     if (workspace && ((uintptr_t)workspace % 256) != 0)
@@ -636,6 +642,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         s->prm.dt_max = grid->real_bits == 64 ? default_dt_max<double>(peds, p, dmin) : default_dt_max<float>(peds, p, dmin);
     }
     s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? (nx % 16 == 0 ? 4 : nx % 2 == 0 ? 3 : 2) : (nx % 4 == 0) ? 1 : 0;
+    if (p->flood_order == 2) s->flood_variant = 5;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -759,6 +766,7 @@ extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
     if (!s) return SIM_EINVAL;
     DeviceGuard on_device(s);
     if (variant < 0 || variant > 4) return fail(s, SIM_EINVAL, "variant must be 0..4");
+    if (s->prm.flood_order == 2) return fail(s, SIM_EINVAL, "flood_order = 2 has one kernel (variant 5)");
     if (variant == 4 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
     if (variant == 3 && s->grid.nx % 2 != 0) return fail(s, SIM_EINVAL, "the two-column march kernel needs nx % 2 == 0");
     if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");
