@@ -45,6 +45,9 @@ class OrcConfig(C.Structure):
         ("layer_thickness", C.c_double), ("t_pick", C.c_double), ("t_drop", C.c_double),
         ("t_end", C.c_double),
         ("flood_order", C.c_int),
+        ("open_sides", C.c_int), ("n_doors", C.c_int), ("door_cells", _ip), ("door_target", _ip),
+        ("spawn_rate", C.c_double), ("target_population", C.c_int), ("spawn_seed", C.c_ulonglong),
+        ("spawn_vpref_lo", C.c_double), ("spawn_vpref_hi", C.c_double), ("pactive0", _bp),
     ]
 
 
@@ -56,6 +59,7 @@ class OrcStats(C.Structure):
         ("clamped_volume", C.c_double),
         ("cursor", C.c_int), ("layer", C.c_int), ("bags", C.c_int), ("barrier_complete", C.c_int),
         ("deposits", C.c_longlong),
+        ("outflow_volume", C.c_double), ("spawned", C.c_longlong), ("triggered", C.c_int),
     ]
 
 
@@ -97,6 +101,8 @@ def lib():
         L.orc_hydrograph.restype = d
         L.orc_social_bruteforce.argtypes = [C.c_int, _dp, _dp, _bp, d, d, d, d, C.c_int, _dp, _dp]
         L.orc_social_bruteforce.restype = None
+        L.orc_philox4x32.argtypes = [C.POINTER(C.c_uint), C.POINTER(C.c_uint), C.POINTER(C.c_uint)]
+        L.orc_philox4x32.restype = None
         L.orc_create.argtypes = [C.POINTER(OrcConfig)]
         L.orc_create.restype = C.c_void_p
         L.orc_destroy.argtypes = [C.c_void_p]
@@ -154,6 +160,15 @@ def face(g, hi, uni, uti, zi, hk, unk, utk, zk):
 
 def minmod(a, b):
     return lib().orc_minmod(a, b)
+
+
+def philox4x32(counter, key):
+    """Philox4x32-10 of the oracle (spawning, D5): 4 + 2 uint32 in, 4 uint32 out."""
+    c = (C.c_uint * 4)(*[int(v) & 0xffffffff for v in counter])
+    k = (C.c_uint * 2)(*[int(v) & 0xffffffff for v in key])
+    out = (C.c_uint * 4)()
+    lib().orc_philox4x32(c, k, out)
+    return [int(v) for v in out]
 
 
 def friction(g, n, dt, h_dry, h, qx, qy):
@@ -254,6 +269,16 @@ class Oracle:
         cfg.layer_thickness, cfg.t_pick, cfg.t_drop = sc.layer_thickness, sc.t_pick, sc.t_drop
         cfg.t_end = sc.t_end
         cfg.flood_order = int(getattr(sc, "flood_order", 1))
+        cfg.open_sides = int(getattr(sc, "open_sides", 0))
+        doors = np.asarray(getattr(sc, "door_cells", np.zeros(0, np.int32)), np.int32)
+        cfg.n_doors = int(len(doors))
+        setp("door_cells", doors, np.int32, _ip)
+        setp("door_target", getattr(sc, "door_target", np.zeros(0, np.int32)), np.int32, _ip)
+        cfg.spawn_rate = float(getattr(sc, "spawn_rate", 0.0))
+        cfg.target_population = int(getattr(sc, "target_population", 0))
+        cfg.spawn_seed = int(getattr(sc, "spawn_seed", 0))
+        cfg.spawn_vpref_lo = float(getattr(sc, "spawn_vpref_lo", 1.0)); cfg.spawn_vpref_hi = float(getattr(sc, "spawn_vpref_hi", 1.4))
+        setp("pactive0", getattr(sc, "pactive0", None), np.uint8, _bp)
         self._h = L.orc_create(C.byref(cfg))
         if not self._h:
             raise ValueError("orc_create failed")

@@ -16,6 +16,10 @@
  * (53 >= 2*24+2), so both sides take those decisions in the same precision.
  *
  * No blocking, fusion or reordering: loops over cells, faces and agents as written.
+ *
+ * Widened scope: flood_step_muscl (8f-2, readings M1-M7) and, for 8f-3 (P:L136, L164,
+ * L180-186; readings D1-D9 of DESIGN.md), open domain edges, entrance doors that let pedestrians
+ * in before the flood, their wandering to a destination door, and the evacuation trigger.
  */
 #include "floodped_oracle.h"
 
@@ -50,6 +54,12 @@ struct orc_sim {
     long long step, deposits, neg_clamps;
     double clamped_volume;
     int cursor, layer, bags, complete;
+    /* SURVEY 8f-3 */
+    int *door_cells, *door_target;
+    double door_credit[16];       /* fractional newcomers owed by each door (D3) */
+    double outflow_volume;
+    long long spawned;
+    int triggered;
 };
 
 static double rnd(const orc_sim *s, double v) { return s->c.real_bits == 32 ? (double)(float)v : v; }
@@ -255,6 +265,69 @@ static void social_from_list(const orc_sim *s, int i, double *ax, double *ay)
         }
 }
 
+/* ------------------------------------------------------------------ trigger, doors */
+
+/* D7 ("Once a positive water depth information is received by any navigation agent"):
+ * a wet cell (h > h_dry, S:8c-C5) exists */
+static int any_wet(const orc_sim *s)
+{
+    for (int c = 0; c < s->ncell; ++c)
+        if (!s->mask[c] && s->h[c] > s->c.h_dry) return 1;
+    return 0;
+}
+
+/* Philox4x32-10, the counter-based generator of Salmon, Moraes, Dror & Shaw (SC'11), written out
+ * from its definition: ten rounds of  (c0,c1,c2,c3) <- (hi(M1 c2)^c1^k0, lo(M1 c2), hi(M0 c0)^c3^k1, lo(M0 c0)),
+ * the key bumped by the Weyl constants after every round but the last. */
+void orc_philox4x32(const unsigned int c[4], const unsigned int k[2], unsigned int out[4])
+{
+    unsigned int c0 = c[0], c1 = c[1], c2 = c[2], c3 = c[3], k0 = k[0], k1 = k[1];
+    for (int r = 0; r < 10; ++r) {
+        unsigned long long p0 = 0xD2511F53ull * c0, p1 = 0xCD9E8D57ull * c2;
+        unsigned int n0 = (unsigned int)(p1 >> 32) ^ c1 ^ k0, n1 = (unsigned int)p1;
+        unsigned int n2 = (unsigned int)(p0 >> 32) ^ c3 ^ k1, n3 = (unsigned int)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* D3-D5: doors let pedestrians in at a constant rate while the population is below its target
+ * (P:L186), each newcomer bound for one of the doors with equal probability */
+static void spawn_step(orc_sim *s, double dt)
+{
+    const orc_config *p = &s->c;
+    int pop = 0;
+    for (int i = 0; i < s->np; ++i) pop += s->active[i] ? 1 : 0;
+    for (int d = 0; d < p->n_doors; ++d) {
+        s->door_credit[d] = s->door_credit[d] + p->spawn_rate * dt;
+        while (s->door_credit[d] >= 1.0) {
+            int slot = -1;
+            if (pop < p->target_population)
+                for (int i = 0; i < s->np; ++i) if (!s->active[i]) { slot = i; break; }   /* lowest free slot (D4) */
+            if (slot < 0) { s->door_credit[d] = 1.0; break; }          /* full: the door waits, owing one */
+            unsigned int ctr[4] = { (unsigned int)(s->spawned & 0xffffffffu), (unsigned int)(s->spawned >> 32), 0u, 0u };
+            unsigned int key[2] = { (unsigned int)(p->spawn_seed & 0xffffffffu), (unsigned int)(p->spawn_seed >> 32) };
+            unsigned int r[4];
+            orc_philox4x32(ctr, key, r);
+            const int dest = (int)(((unsigned long long)r[0] * (unsigned long long)p->n_doors) >> 32);
+            const double ux = (double)r[1] * (1.0 / 4294967296.0), uy = (double)r[2] * (1.0 / 4294967296.0);
+            const double uv = (double)r[3] * (1.0 / 4294967296.0);
+            const int ci = s->door_cells[d] % p->nx, cj = s->door_cells[d] / p->nx;
+            /* inside the door cell, 10 % away from its edges */
+            s->x[slot] = rnd(s, (((double)ci + 0.1) + 0.8 * ux) * p->dx);
+            s->y[slot] = rnd(s, (((double)cj + 0.1) + 0.8 * uy) * p->dy);
+            s->vx[slot] = 0.0; s->vy[slot] = 0.0; s->timer[slot] = 0.0;
+            s->vpref[slot] = rnd(s, p->spawn_vpref_lo + (p->spawn_vpref_hi - p->spawn_vpref_lo) * uv);
+            s->role[slot] = 0; s->state[slot] = ORC_DRY;
+            s->fsm[slot] = (unsigned char)(ORC_WANDER + dest);
+            s->active[slot] = 1;
+            s->cell[slot] = s->door_cells[d];
+            s->door_credit[d] -= 1.0; s->spawned += 1; pop += 1;
+        }
+    }
+}
+
 /* ------------------------------------------------------------------ create / destroy */
 
 orc_sim *orc_create(const orc_config *cfg)
@@ -292,6 +365,8 @@ orc_sim *orc_create(const orc_config *cfg)
     s->nav_dir = dup_mem(cfg->nav_dir, (size_t)cfg->n_targets * (size_t)nc);
     s->exit_cells = dup_mem(cfg->exit_cells, (size_t)cfg->n_exit_cells * sizeof(int));
     s->line_cells = dup_mem(cfg->line_cells, (size_t)cfg->n_line * sizeof(int));
+    s->door_cells = dup_mem(cfg->door_cells, (size_t)cfg->n_doors * sizeof(int));
+    s->door_target = dup_mem(cfg->door_target, (size_t)cfg->n_doors * sizeof(int));
 
     int np = s->np = cfg->n_peds;
     size_t pb = (size_t)np * sizeof(double);
@@ -307,7 +382,7 @@ orc_sim *orc_create(const orc_config *cfg)
     s->active = dup_mem(NULL, (size_t)np); s->active1 = dup_mem(NULL, (size_t)np);
     s->cell = dup_mem(NULL, (size_t)np * sizeof(int));
     for (int i = 0; i < np; ++i) {
-        s->active[i] = 1;
+        s->active[i] = cfg->pactive0 ? (cfg->pactive0[i] != 0) : 1;
         s->fsm[i] = s->role[i] ? ORC_TO_STORAGE : ORC_EVACUATE;   /* P:L140 */
         s->cell[i] = cell_iy(s, s->y[i]) * cfg->nx + cell_ix(s, s->x[i]);
     }
@@ -333,6 +408,7 @@ orc_sim *orc_create(const orc_config *cfg)
     s->complete = (cfg->n_line <= 0 || cfg->n_layers <= 0) ? 1 : 0;
     s->dt = next_dt(s, s->h, s->qx, s->qy);
     if (s->t + s->dt > s->c.t_end) s->dt = fmax(0.0, s->c.t_end - s->t);
+    s->triggered = any_wet(s);                                  /* D8 */
     return s;
 }
 
@@ -344,7 +420,7 @@ void orc_destroy(orc_sim *s)
         s->inflow_cell, s->inflow_side, s->hydro_t, s->hydro_q, s->nav_dir, s->exit_cells,
         s->line_cells, s->x, s->y, s->vx, s->vy, s->vpref, s->timer, s->x1, s->y1, s->vx1, s->vy1,
         s->timer1, s->role, s->state, s->fsm, s->active, s->state1, s->fsm1, s->active1, s->cell,
-        s->head, s->next };
+        s->head, s->next, s->door_cells, s->door_target };
     for (size_t k = 0; k < sizeof p / sizeof p[0]; ++k) free(p[k]);
     for (int f = 0; f < 4; ++f) for (int k = 0; k < 4; ++k) free(s->fv[f][k]);
     free(s);
@@ -355,12 +431,27 @@ void orc_destroy(orc_sim *s)
 /* state of the neighbour across one face of cell c: the cell itself if it is an interior
  * walkable cell, else the wall ghost (S:8c-O2.1): same h and z, normal velocity
  * negated, tangential kept */
+/* D1: is the face of cell c = (i, j) towards (di, dj) an OPEN domain-edge face?  The side must be
+ * flagged open and the face must not be an inflow face (those stay walls for momentum, C14). */
+static int open_face(const orc_sim *s, int c, int i, int j, int di, int dj)
+{
+    int side;
+    if (di < 0 && i == 0) side = ORC_W;
+    else if (di > 0 && i == s->c.nx - 1) side = ORC_E;
+    else if (dj < 0 && j == 0) side = ORC_S;
+    else if (dj > 0 && j == s->c.ny - 1) side = ORC_N;
+    else return 0;
+    return ((s->c.open_sides >> side) & 1) && s->inflow_mult[side][c] == 0;
+}
+
 static void neighbour(const orc_sim *s, int c, int i, int j, int di, int dj,
                       double hc, double unc, double utc, double zc,
                       double *hk, double *unk, double *utk, double *zk)
 {
     int ii = i + di, jj = j + dj;
     int wall = (ii < 0 || jj < 0 || ii >= s->c.nx || jj >= s->c.ny);
+    /* D1: an open domain edge has a transmissive ghost (zero gradient: the cell's own state) */
+    if (wall && open_face(s, c, i, j, di, dj)) { *hk = hc; *unk = unc; *utk = utc; *zk = zc; return; }
     int k = wall ? c : jj * s->c.nx + ii;
     if (!wall && s->mask[k]) wall = 1;
     if (wall) { *hk = hc; *unk = -unc; *utk = utc; *zk = zc; return; }
@@ -404,6 +495,12 @@ static void flood_step(orc_sim *s, double q_in)
             FE0 -= q_in * s->inflow_mult[ORC_E][c];
             GS0 += q_in * s->inflow_mult[ORC_S][c];
             GN0 -= q_in * s->inflow_mult[ORC_N][c];
+
+            /* volume leaving through open edge faces (D1) */
+            if (open_face(s, c, i, j, +1, 0)) s->outflow_volume += dt * FE0 * dy;
+            if (open_face(s, c, i, j, -1, 0)) s->outflow_volume -= dt * FW0 * dy;
+            if (open_face(s, c, i, j, 0, +1)) s->outflow_volume += dt * GN0 * dx;
+            if (open_face(s, c, i, j, 0, -1)) s->outflow_volume -= dt * GS0 * dx;
 
             /* Eq. (2) */
             double hn  = h        - dt / dx * (FE0 - FW0) - dt / dy * (GN0 - GS0);
@@ -533,7 +630,8 @@ static void flood_step_muscl(orc_sim *s, double q_in)
                 const int di = (f == ORC_E) - (f == ORC_W), dj = (f == ORC_N) - (f == ORC_S);
                 double hi, uni, uti, zi, hk, unk, utk, zk, F[3], Fi, Fk;
                 muscl_face_state(s, c, f, &hi, &uni, &uti, &zi);
-                if (is_wall(s, i + di, j + dj)) { hk = hi; unk = -uni; utk = uti; zk = zi; }   /* wall ghost (S:8c-O2.1) */
+                if (open_face(s, c, i, j, di, dj)) { hk = hi; unk = uni; utk = uti; zk = zi; }  /* transmissive ghost (D1) */
+                else if (is_wall(s, i + di, j + dj)) { hk = hi; unk = -uni; utk = uti; zk = zi; }   /* wall ghost (S:8c-O2.1) */
                 else muscl_face_state(s, (j + dj) * nx + (i + di), f ^ 1, &hk, &unk, &utk, &zk);
                 if (f == ORC_E || f == ORC_N) { orc_face(g, hi, uni, uti, zi, hk, unk, utk, zk, F, &Fi, &Fk); }
                 else                          { orc_face(g, hk, unk, utk, zk, hi, uni, uti, zi, F, &Fk, &Fi); }
@@ -545,6 +643,10 @@ static void flood_step_muscl(orc_sim *s, double q_in)
             F0[ORC_E] -= q_in * s->inflow_mult[ORC_E][c];
             F0[ORC_S] += q_in * s->inflow_mult[ORC_S][c];
             F0[ORC_N] -= q_in * s->inflow_mult[ORC_N][c];
+            if (open_face(s, c, i, j, +1, 0)) s->outflow_volume += dt * F0[ORC_E] * dy;
+            if (open_face(s, c, i, j, -1, 0)) s->outflow_volume -= dt * F0[ORC_W] * dy;
+            if (open_face(s, c, i, j, 0, +1)) s->outflow_volume += dt * F0[ORC_N] * dx;
+            if (open_face(s, c, i, j, 0, -1)) s->outflow_volume -= dt * F0[ORC_S] * dx;
             /* M5: centred bed-slope source of the cell's own (predicted) face values */
             const double Sx = 0.5 * g * (hf[ORC_W] + hf[ORC_E]) * (zf[ORC_W] - zf[ORC_E]) / dx;
             const double Sy = 0.5 * g * (hf[ORC_S] + hf[ORC_N]) * (zf[ORC_S] - zf[ORC_N]) / dy;
@@ -577,6 +679,7 @@ static long long ped_step(orc_sim *s)
     const orc_config *p = &s->c;
     const double dt = s->dt;
     const int complete0 = s->complete;           /* value at the start of the step (S:8c-O3.7) */
+    const int triggered0 = s->triggered;         /* likewise (D7) */
     long long D = 0;
     build_cell_list(s);
     for (int i = 0; i < s->np; ++i) {
@@ -587,6 +690,12 @@ static long long ped_step(orc_sim *s)
         /* 1. containing cell, sample U^n there (S:8c-C19, C20) */
         int c = s->cell[i];
         int fsm = s->fsm[i];
+        /* D7: once water is in the domain, those still wandering become evacuees */
+        if (fsm >= ORC_WANDER && triggered0) { fsm = ORC_EVACUATE; s->fsm1[i] = ORC_EVACUATE; }
+        /* D6: a wanderer leaves through its destination door */
+        if (fsm >= ORC_WANDER) {
+            if (cheb(s, c, s->door_cells[fsm - ORC_WANDER]) <= p->arrive_cells) { s->active1[i] = 0; continue; }
+        } else
         /* 8. exit (S:8c-C29): evaluated on the level-n cell */
         if (s->role[i] == 0 || fsm == ORC_EVACUATE) {
             int out = 0;
@@ -607,6 +716,7 @@ static long long ped_step(orc_sim *s)
         int target = p->exit_target;
         if (fsm == ORC_TO_STORAGE) target = p->storage_target;
         else if (fsm == ORC_TO_BARRIER) target = p->drop_target;
+        else if (fsm >= ORC_WANDER) target = s->door_target[fsm - ORC_WANDER];
         double ex, ey;
         dir_vector(s->nav_dir[(size_t)target * s->ncell + c], &ex, &ey);
         /* 4. social repulsion from agents in adjacent bins (S:8c-C24, C26) */
@@ -689,8 +799,12 @@ int orc_step(orc_sim *s, long long n)
         tb = s->fsm; s->fsm = s->fsm1; s->fsm1 = tb;
         tb = s->active; s->active = s->active1; s->active1 = tb;
         /* O5 */
+        const double dt_taken = s->dt;
         s->t += s->dt;
         s->step += 1;
+        /* D7: trigger on U^{n+1}; D3: doors let newcomers in (they exist from level n+1 on) */
+        if (!s->triggered && any_wet(s)) s->triggered = 1;
+        if (!s->triggered && s->c.n_doors > 0) spawn_step(s, dt_taken);
         s->dt = next_dt(s, s->h, s->qx, s->qy);
         if (s->t + s->dt > s->c.t_end) s->dt = fmax(0.0, s->c.t_end - s->t);
     }
@@ -719,6 +833,7 @@ void orc_get_stats(orc_sim *s, orc_stats *o)
     o->neg_depth_clamps = s->neg_clamps; o->clamped_volume = s->clamped_volume;
     o->cursor = s->cursor; o->layer = s->layer; o->bags = s->bags;
     o->barrier_complete = s->complete; o->deposits = s->deposits;
+    o->outflow_volume = s->outflow_volume; o->spawned = s->spawned; o->triggered = s->triggered;
 }
 
 void orc_read_flood(orc_sim *s, double *h, double *u, double *v, double *z, double *hr)
@@ -798,6 +913,7 @@ void orc_write_flood(orc_sim *s, const double *h, const double *qx, const double
     if (qx) memcpy(s->qx, qx, nb);
     if (qy) memcpy(s->qy, qy, nb);
     if (z) memcpy(s->z, z, nb);
+    if (!s->triggered && any_wet(s)) s->triggered = 1;       /* D8 */
 }
 
 void orc_write_peds(orc_sim *s, const double *x, const double *y, const double *vx, const double *vy,

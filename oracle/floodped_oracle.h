@@ -79,7 +79,22 @@ typedef struct {
     /* ---- widened scope; zero-initialised = the paper's first-order closed-wall scheme ---- */
     int flood_order;             /* 0 or 1: first order ("reduced to first-order accuracy");
                                     2: MUSCL-Hancock, the second-order scheme it was reduced from (M1-M7) */
+    /* SURVEY 8f-3 (readings D1-D9 of DESIGN.md): open boundary, entrance
+     * doors with spawning, pre-flood wandering, evacuation trigger */
+    int open_sides;              /* bit (1 << ORC_W/E/S/N): that domain edge is open (transmissive ghost) except at inflow faces (D1) */
+    int n_doors;                 /* entrance doors (7, "equal probability of 1/7"), at most 16 */
+    const int *door_cells;       /* [n_doors] walkable cell of each door */
+    const int *door_target;      /* [n_doors] index of the navigation field that leads to it */
+    double spawn_rate;           /* pedestrians entering per second per door ("constant rate of 10 ... per entrance") (D3) */
+    int target_population;       /* doors spawn only while fewer pedestrians are active ("maintain a total of 1000") */
+    unsigned long long spawn_seed;     /* key of the counter-based generator (Philox4x32-10) that draws a newcomer (D5) */
+    double spawn_vpref_lo, spawn_vpref_hi;   /* dry walking speed of a newcomer, uniform in [lo, hi) */
+    const unsigned char *pactive0;     /* [n_peds] initial active flag per slot, NULL = all active; inactive slots are free for newcomers */
 } orc_config;
+
+/* pedestrians that entered through a door and walk to a destination door before the flood
+ * (P:L164, L186): fsm = ORC_WANDER + destination door; they become evacuees at the trigger */
+enum { ORC_WANDER = 8 };
 
 typedef struct {
     double t, dt;
@@ -90,6 +105,9 @@ typedef struct {
     double clamped_volume;
     int cursor, layer, bags, barrier_complete;
     long long deposits;
+    double outflow_volume;       /* volume that left through open edges (D1): V = V0 + inflow - outflow + clamped */
+    long long spawned;           /* newcomers so far (D3) */
+    int triggered;               /* 1 once a wet cell exists: no more entries, everybody evacuates (D7) */
 } orc_stats;
 
 typedef struct orc_sim orc_sim;
@@ -124,6 +142,9 @@ double orc_hydrograph(int n, const double *t, const double *q, double time);
 void orc_social_bruteforce(int n, const double *x, const double *y, const unsigned char *active,
                            double A_s, double B_s, double radius, double R_int,
                            int i, double *ax, double *ay);
+
+/* Philox4x32-10 (Salmon et al. 2011): counter c[4], key k[2] -> out[4] (D5) */
+void orc_philox4x32(const unsigned int c[4], const unsigned int k[2], unsigned int out[4]);
 
 /* ---- the simulator ---- */
 orc_sim *orc_create(const orc_config *cfg);

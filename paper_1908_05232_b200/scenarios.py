@@ -87,6 +87,16 @@ class Scenario:
     steps: int = 0                           # the run length the config names (0: until t_end)
     # widened scope
     flood_order: int = 1                     # 1: the paper's first-order scheme; 2: MUSCL-Hancock (8f-2)
+    # 8f-3 (D1-D9): open edges, entrance doors, pre-flood phase, trigger
+    open_sides: int = 0                      # bit 0 W, 1 E, 2 S, 3 N: that domain edge is open (transmissive)
+    door_cells: np.ndarray = field(default_factory=lambda: np.zeros(0, np.int32))
+    door_target: np.ndarray = field(default_factory=lambda: np.zeros(0, np.int32))   # nav field index per door
+    spawn_rate: float = 0.0                  # pedestrians per second per door
+    target_population: int = 0
+    spawn_seed: int = 0
+    spawn_vpref_lo: float = 1.0
+    spawn_vpref_hi: float = 1.4
+    pactive0: np.ndarray | None = None       # initial active flag per slot (None: all active)
 
     @property
     def real(self):
@@ -356,6 +366,52 @@ def shopping_centre(n: int = 256, n_evac: int = 2000, n_resp: int = 0, q_peak: f
         sc.bags_per_cell_layer, sc.n_layers, sc.layer_thickness = 1, 12, 0.05
         sc.t_pick = sc.t_drop = 30.0
     return sc
+
+
+def door_hall(n: int = 64, slots: int = 400, n_init: int = 0, target_population: int = 200,
+              spawn_rate: float = 10.0 / 60.0, t_pre: float = 300.0, q_peak: float = 1.0,
+              t_end: float = 1800.0, seed: int = 7, open_north: bool = False, real_bits: int = 32) -> Scenario:
+    """Scenario 1 of the paper in miniature (Fig. 4 unreadable, so the
+    geometry is synthetic): an n x n hall at 0.5 m * 256/n with the walls and bed of the shopping
+    centre, SEVEN entrance doors (three on the west wall, three on the east, one on the south), a
+    pre-flood phase of `t_pre` seconds during which pedestrians enter at `spawn_rate` per second and
+    door, each bound for one of the seven doors with probability 1/7, then the triangular flood
+    through the southern breach; the emergency exit is at the middle of the north wall.  `slots`
+    agent slots, the first `n_init` of them already walking at t = 0."""
+    nx = ny = n
+    s = n / 256.0
+    dx = 0.5 / s
+    mask, z, _ = _hall(n, seed)
+    m = mask.reshape(-1)
+    exit_cell = (ny - 1) * nx + nx // 2
+    i0, i1 = int(round(90 * s)), int(round(166 * s))
+    inflow_cell = np.arange(i0, i1, dtype=np.int32)
+    doors = [(0, ny // 4), (0, ny // 2), (0, 3 * ny // 4), (nx - 1, ny // 4), (nx - 1, ny // 2), (nx - 1, 3 * ny // 4),
+             (max(i0 - 4, 1), 0)]
+    door_cells = np.array([j * nx + i for i, j in doors], np.int32)
+    m[inflow_cell] = 0; m[exit_cell] = 0; m[door_cells] = 0
+    nav_exit, dist = nav_field(mask, [exit_cell])
+    assert np.all(np.isfinite(dist.reshape(-1)[door_cells])), "a door cannot reach the exit"
+    navs = [nav_exit] + [nav_field(mask, [int(c)])[0] for c in door_cells]
+    reachable = np.flatnonzero(np.isfinite(dist.reshape(-1)) & (m == 0))
+    rng = np.random.Generator(np.random.PCG64(100 + seed))
+    x, y = _place_in_cells(rng, reachable, nx, dx, dx, slots)
+    vpref = _vpref(rng, slots)
+    act = np.zeros(slots, np.uint8); act[:n_init] = 1
+    ht, hq = _triangle(t_pre, t_pre + 300.0, t_pre + 600.0, q_peak)
+    return Scenario(
+        name="door_hall", nx=nx, ny=ny, dx=dx, dy=dx, real_bits=real_bits,
+        z=_as_real(z.reshape(-1), real_bits), manning=_as_real(np.full(nx * ny, 0.01), real_bits),
+        mask=m.copy(), h0=np.zeros(nx * ny, np.float32 if real_bits == 32 else np.float64), u0=None, v0=None,
+        px=_keep_inside(x, nx, dx, real_bits), py=_keep_inside(y, ny, dx, real_bits),
+        pvx=np.zeros(slots), pvy=np.zeros(slots), pvpref=_as_real(vpref, real_bits), prole=np.zeros(slots, np.uint8),
+        nav_dir=np.stack(navs), exit_cells=np.array([exit_cell], np.int32), exit_target=0,
+        inflow_cell=inflow_cell, inflow_side=np.full(inflow_cell.shape, SIDE_S, np.uint8),
+        hydro_t=ht, hydro_q=hq, t_end=t_end,
+        open_sides=(1 << SIDE_N) if open_north else 0,
+        door_cells=door_cells, door_target=np.arange(1, 8, dtype=np.int32),
+        spawn_rate=spawn_rate, target_population=target_population, spawn_seed=0x5eed0000 + seed,
+        spawn_vpref_lo=1.0, spawn_vpref_hi=1.4, pactive0=act)
 
 
 def pre_flood_intervention(n: int = 256, n_evac: int = 1000, n_resp: int = 100,
