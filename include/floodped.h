@@ -69,6 +69,9 @@ extern "C" {
 #define SIM_FSM_PICKING 2
 #define SIM_FSM_TO_BARRIER 3
 #define SIM_FSM_DROPPING 4
+/* entered through a door before the flood and walking to destination door d: SIM_FSM_WANDER + d
+ * (P:L164, L186); becomes SIM_FSM_EVACUATE at the trigger */
+#define SIM_FSM_WANDER 8
 /* navigation direction codes: 0..7 = E,NE,N,NW,W,SW,S,SE */
 #define SIM_DIR_NONE 255
 
@@ -90,6 +93,8 @@ typedef struct {                                /* pedestrian agents (P:L83, L13
     int32_t        n;
     const void    *x, *y, *vx, *vy, *v_pref;    /* [n] real; v_pref = dry walking speed */
     const uint8_t *role;                        /* [n] 0 evacuee, 1 responder             */
+    const uint8_t *active;                      /* [n] 1 = in the domain at t = 0; NULL = everybody.  Inactive slots are
+                                                   free for newcomers   */
 } sim_peds_t;
 
 typedef struct {
@@ -125,6 +130,17 @@ typedef struct {
      * M1-M7 of DESIGN.md): minmod slopes, Hancock half-step predictor, same HLLC flux, hydrostatic
      * reconstruction, friction and CFL rule */
     int32_t flood_order;
+    /* open edges, entrance doors, pre-flood phase, evacuation trigger (P:L136, L164,
+     * L180-186; readings D1-D9 of DESIGN.md).  All zero = the closed hall of the five configs. */
+    int32_t        open_sides;                  /* bit (1 << SIM_SIDE_*): that domain edge is open (transmissive ghost) except at
+                                                   inflow faces (D1); the flood kernel is then variant 0 (or 5 with flood_order 2) */
+    int32_t        n_doors;                     /* entrance doors, at most 16 (seven, probability 1/7 each)       */
+    const int32_t *door_cells;                  /* [n_doors] walkable cell of each door                                   */
+    const int32_t *door_target;                 /* [n_doors] navigation field (index into nav_dir) that leads to it       */
+    double         spawn_rate;                  /* pedestrians entering per second and door while not triggered  */
+    int32_t        target_population;           /* doors let somebody in only while fewer pedestrians are active */
+    uint64_t       spawn_seed;                  /* key of the Philox4x32-10 draws of a newcomer (D5)                      */
+    double         spawn_vpref_lo, spawn_vpref_hi;   /* dry walking speed of a newcomer: uniform in [lo, hi)              */
 } sim_params_t;
 
 typedef struct {
@@ -136,6 +152,9 @@ typedef struct {
     double  clamped_volume;
     int32_t cursor, layer, bags, barrier_complete;
     int64_t deposits;
+    double  outflow_volume;                     /* left through open edges (D1): V = V0 + inflow - outflow + clamped */
+    int64_t spawned;                            /* newcomers so far (D3)                  */
+    int32_t triggered;                          /* 1 once a wet cell exists (D7)  */
 } sim_stats_t;
 
 /* Bytes of device workspace sim_create needs for this problem. */
@@ -181,6 +200,9 @@ int sim_write_peds(sim_t *s, const void *x, const void *y, const void *vx, const
                    const uint8_t *fsm, const uint8_t *active, const void *timer);
 int sim_set_time(sim_t *s, double t, double dt);
 int sim_set_barrier(sim_t *s, int32_t cursor, int32_t layer, int32_t bags, int32_t complete);
+/* The device's Philox4x32-10 (D5) on n (counter[4], key[2]) rows of `in` -> n rows of 4 words in
+ * `out`; HOST pointers; s only names the device and stream. */
+int sim_test_philox(sim_t *s, const uint32_t *in, uint32_t *out, int32_t n);
 /* Choose the flood kernel: 0 = one thread per cell, 4 faces each (any nx); 1 = 64x16 tiles, each
  * face once, shared-memory staging (nx % 4 == 0); 2 = row-marching strips of 256 columns, each
  * face once, rows prefetched in registers (any nx); 3 = as 2 with two columns per thread and

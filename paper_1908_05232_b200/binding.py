@@ -19,7 +19,7 @@ SIM_OK, SIM_EINVAL, SIM_ENOMEM, SIM_ECUDA, SIM_ENOTFINITE = 0, -1, -2, -3, -4
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
-    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap",
+    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap",
     "sim_kernels_per_step", "sim_last_error", "sim_destroy",
 ]
 
@@ -40,7 +40,7 @@ class SimTopo(C.Structure):
 
 class SimPeds(C.Structure):
     _fields_ = [("n", C.c_int32), ("x", _vp), ("y", _vp), ("vx", _vp), ("vy", _vp), ("v_pref", _vp),
-                ("role", _u8p)]
+                ("role", _u8p), ("active", _u8p)]
 
 
 class SimParams(C.Structure):
@@ -61,6 +61,9 @@ class SimParams(C.Structure):
         ("layer_thickness", C.c_double), ("t_pick", C.c_double), ("t_drop", C.c_double),
         ("t_end", C.c_double),
         ("flood_order", C.c_int32),
+        ("open_sides", C.c_int32), ("n_doors", C.c_int32), ("door_cells", _i32p), ("door_target", _i32p),
+        ("spawn_rate", C.c_double), ("target_population", C.c_int32), ("spawn_seed", C.c_uint64),
+        ("spawn_vpref_lo", C.c_double), ("spawn_vpref_hi", C.c_double),
     ]
 
 
@@ -71,6 +74,7 @@ class SimStats(C.Structure):
         ("hist", C.c_int64 * 6), ("neg_depth_clamps", C.c_int64), ("clamped_volume", C.c_double),
         ("cursor", C.c_int32), ("layer", C.c_int32), ("bags", C.c_int32), ("barrier_complete", C.c_int32),
         ("deposits", C.c_int64),
+        ("outflow_volume", C.c_double), ("spawned", C.c_int64), ("triggered", C.c_int32),
     ]
 
 
@@ -109,6 +113,7 @@ def load_library(path: str = LIB_PATH):
     L.sim_write_peds.argtypes = [_vp] * 8
     L.sim_set_time.argtypes = [_vp, C.c_double, C.c_double]
     L.sim_set_barrier.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32]
+    L.sim_test_philox.argtypes = [_vp, _vp, _vp, C.c_int32]
     L.sim_set_flood_variant.argtypes = [_vp, C.c_int32]
     L.sim_get_flood_variant.argtypes = [_vp]
     L.sim_set_march_rows.argtypes = [_vp, C.c_int32]
@@ -155,7 +160,8 @@ class _Marshalled:
         n = int(sc.px.shape[0])
         self.peds = SimPeds(n, _np_ptr(arr(sc.px, real)), _np_ptr(arr(sc.py, real)),
                             _np_ptr(arr(sc.pvx, real)), _np_ptr(arr(sc.pvy, real)),
-                            _np_ptr(arr(sc.pvpref, real)), typed(sc.prole, np.uint8, _u8p))
+                            _np_ptr(arr(sc.pvpref, real)), typed(sc.prole, np.uint8, _u8p),
+                            typed(getattr(sc, "pactive0", None), np.uint8, _u8p))
         p = SimParams()
         p.g, p.cfl, p.dt_max, p.h_dry = sc.g, sc.cfl, sc.dt_max, sc.h_dry
         p.couple_roughness, p.n_cap = sc.couple_roughness, sc.n_cap
@@ -180,6 +186,15 @@ class _Marshalled:
         p.bags_per_cell_layer, p.n_layers = sc.bags_per_cell_layer, sc.n_layers
         p.layer_thickness, p.t_pick, p.t_drop, p.t_end = sc.layer_thickness, sc.t_pick, sc.t_drop, sc.t_end
         p.flood_order = int(getattr(sc, "flood_order", 1))
+        p.open_sides = int(getattr(sc, "open_sides", 0))
+        doors = getattr(sc, "door_cells", np.zeros(0, np.int32))
+        p.n_doors = len(doors)
+        p.door_cells = typed(doors, np.int32, _i32p)
+        p.door_target = typed(getattr(sc, "door_target", np.zeros(0, np.int32)), np.int32, _i32p)
+        p.spawn_rate = float(getattr(sc, "spawn_rate", 0.0))
+        p.target_population = int(getattr(sc, "target_population", 0))
+        p.spawn_seed = int(getattr(sc, "spawn_seed", 0))
+        p.spawn_vpref_lo = float(getattr(sc, "spawn_vpref_lo", 1.0)); p.spawn_vpref_hi = float(getattr(sc, "spawn_vpref_hi", 1.4))
         self.params = p
 
 
@@ -324,6 +339,13 @@ class Sim:
 
     def set_time(self, t, dt):
         self._chk(self._L.sim_set_time(self._h, float(t), float(dt)))
+
+    def philox(self, counters_keys):
+        """the device's Philox4x32-10 on rows of (c0, c1, c2, c3, k0, k1)"""
+        a = np.ascontiguousarray(counters_keys, np.uint32).reshape(-1, 6)
+        out = np.empty((a.shape[0], 4), np.uint32)
+        self._chk(self._L.sim_test_philox(self._h, _np_ptr(a), _np_ptr(out), a.shape[0]))
+        return out
 
     def set_barrier(self, cursor, layer, bags, complete):
         self._chk(self._L.sim_set_barrier(self._h, int(cursor), int(layer), int(bags), int(complete)))

@@ -26,6 +26,10 @@ struct Ctl {
     unsigned int scan_epoch;         // makes the look-back flags of the scan self-resetting
     unsigned int scan_ticket;        // dynamic tile index of the scan
     int occ_next;                    // N_p buffer the binning chain of the NEXT step fills (= parity ^ 1), published by the pedestrian step
+    // SURVEY 8f-3 (D1-D9)
+    double outflow_volume;           // volume that left through open edges (D1)
+    long long spawned;               // newcomers let in by the doors so far (D3); also the Philox counter (D5)
+    int triggered;                   // a wet cell has been seen: no more entries, everybody evacuates (D7)
     float pair_c1, pair_c2;          // fp32 pair force A_s e^{(2r-d)/B_s} = 2^{c1 + c2 d}: read from memory once per thread so that they
                                      // stay in registers (as kernel parameters ptxas reloads them from the constant bank per candidate)
 };

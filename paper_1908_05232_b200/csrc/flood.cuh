@@ -35,8 +35,24 @@ struct FloodArgs {
     const T *ghost_zero, *ghost_inf;  // one strip-wide row of zeros / of +inf, and of zero bytes: the row beyond the
     const uint8_t *ghost_occ;         // domain edge as the TMA kernel loads it (a wall = a row of solid cells, C13)
     int R;                            // march kernel: rows per chunk
+    int open_sides;                   // bit per domain edge (W, E, S, N): open, transmissive ghost; kernels 0 and 5 only
     Ctl *ctl;
 };
+
+// D1: is the domain-edge face of cell (i, j) on `side` open?  Inflow faces stay inflow faces (C14).
+template <typename T>
+__device__ __forceinline__ bool open_face(const FloodArgs<T> &a, int side, int i, int j)
+{
+    return ((a.open_sides >> side) & 1) && a.inflow[side][side < 2 ? j : i] == 0;
+}
+
+// volume leaving through an open face this step (D1): V = V0 + inflow - outflow + clamped
+template <typename T>
+__device__ __forceinline__ void add_outflow(const FloodArgs<T> &a, T dt, T flux_out, T inv_len_other)
+{
+    // face length = cell_area * (1 / the other side's length)
+    atomicAdd(&a.ctl->outflow_volume, (double)dt * (double)flux_out * ((double)a.cell_area * (double)inv_len_other));
+}
 
 // ------------------------------------------------------------------------------------------------
 // HLLC flux on already reconstructed states.  Two-rarefaction wave-speed estimates with the
@@ -160,28 +176,34 @@ __global__ void __launch_bounds__(256) flood_cell_kernel(FloodArgs<T> a)
         if (!is_solid(z)) {
             const T h = H[c], qx = QX[c], qy = QY[c];
             T u, v; primitives(h, qx, qy, a.h_dry, u, v);
-            auto nb = [&](int ii, int jj, T &hk, T &uk, T &vk, T &zk) {
+            const bool oW = i == 0 && open_face(a, 0, i, j), oE = i == a.nx - 1 && open_face(a, 1, i, j);
+            const bool oS = j == 0 && open_face(a, 2, i, j), oN = j == a.ny - 1 && open_face(a, 3, i, j);
+            auto nb = [&](int ii, int jj, bool open, T &hk, T &uk, T &vk, T &zk) {
                 zk = solid_z<T>(); hk = uk = vk = T(0);
                 if (ii >= 0 && jj >= 0 && ii < a.nx && jj < a.ny) {
                     const int k = jj * a.nx + ii;
                     zk = Z[k];
                     if (!is_solid(zk)) { hk = H[k]; primitives(hk, QX[k], QY[k], a.h_dry, uk, vk); }
-                }
+                } else if (open) { hk = h; uk = u; vk = v; zk = z; }       // transmissive ghost (D1)
             };
             T hk, uk, vk, zk, f1L, f1R;
             T FE0, FE1, FE2, FW0, FW1, FW2, GN0, GN1, GN2, GS0, GS1, GS2;
-            nb(i + 1, j, hk, uk, vk, zk);
+            nb(i + 1, j, oE, hk, uk, vk, zk);
             face_flux(a.g, h, u, v, z, hk, uk, vk, zk, FE0, f1L, f1R, FE2); FE1 = f1L;
-            nb(i - 1, j, hk, uk, vk, zk);
+            nb(i - 1, j, oW, hk, uk, vk, zk);
             face_flux(a.g, hk, uk, vk, zk, h, u, v, z, FW0, f1L, f1R, FW2); FW1 = f1R;
-            nb(i, j + 1, hk, uk, vk, zk);
+            nb(i, j + 1, oN, hk, uk, vk, zk);
             face_flux(a.g, h, v, u, z, hk, vk, uk, zk, GN0, f1L, f1R, GN1); GN2 = f1L;
-            nb(i, j - 1, hk, uk, vk, zk);
+            nb(i, j - 1, oS, hk, uk, vk, zk);
             face_flux(a.g, hk, vk, uk, zk, h, v, u, z, GS0, f1L, f1R, GS1); GS2 = f1R;
             if (i == 0) FW0 += qin * T(a.inflow[0][j]);
             if (i == a.nx - 1) FE0 -= qin * T(a.inflow[1][j]);
             if (j == 0) GS0 += qin * T(a.inflow[2][i]);
             if (j == a.ny - 1) GN0 -= qin * T(a.inflow[3][i]);
+            if (oE) add_outflow(a, dt, FE0, a.inv_dx);
+            if (oW) add_outflow(a, dt, -FW0, a.inv_dx);
+            if (oN) add_outflow(a, dt, GN0, a.inv_dy);
+            if (oS) add_outflow(a, dt, -GS0, a.inv_dy);
             finish_cell(a, dt, h, qx, qy, FE0 - FW0, FE1 - FW1, FE2 - FW2, GN0 - GS0, GN1 - GS1, GN2 - GS2,
                         a.n0[c], (int)OCC[c], hn, qxn, qyn, lam);
         }

@@ -137,6 +137,7 @@ __global__ void __launch_bounds__(MTX * MTY) flood_muscl_kernel(FloodArgs<T> a)
         if (s.wet[py][px] != 2) {
             const bool wet = s.wet[py][px] == 1;
             T F0[4], Fn[4], Ft[4], hf[4], zf[4];
+            bool open[4];
 #pragma unroll
             for (int f = 0; f < 4; ++f) {
                 const int di = (f == 1) - (f == 0), dj = (f == 3) - (f == 2);
@@ -145,7 +146,10 @@ __global__ void __launch_bounds__(MTX * MTY) flood_muscl_kernel(FloodArgs<T> a)
                 const T uni = f < 2 ? ui : vi, uti = f < 2 ? vi : ui;
                 T hk = hi, unk = -uni, utk = uti, zk = zi;                   // wall ghost (O2.1)
                 const int wk = s.wet[py + dj][px + di];
-                if (wk != 2) {
+                const bool edge = f == 0 ? i == 0 : f == 1 ? i == a.nx - 1 : f == 2 ? j == 0 : j == a.ny - 1;
+                open[f] = edge && open_face(a, f, i, j);
+                if (open[f]) unk = uni;                                      // transmissive ghost (D1)
+                else if (wk != 2) {
                     const int g = f ^ 1;
                     hk = s.fv[g][0][py + dj][px + di]; zk = s.fv[g][3][py + dj][px + di];
                     const T uk = face_vel(wk == 1, s.fv[g][1][py + dj][px + di], hk, a.h_dry);
@@ -162,6 +166,10 @@ __global__ void __launch_bounds__(MTX * MTY) flood_muscl_kernel(FloodArgs<T> a)
             if (i == a.nx - 1) F0[1] -= qin * T(a.inflow[1][j]);
             if (j == 0) F0[2] += qin * T(a.inflow[2][i]);
             if (j == a.ny - 1) F0[3] -= qin * T(a.inflow[3][i]);
+            if (open[1]) add_outflow(a, dt, F0[1], a.inv_dx);
+            if (open[0]) add_outflow(a, dt, -F0[0], a.inv_dx);
+            if (open[3]) add_outflow(a, dt, F0[3], a.inv_dy);
+            if (open[2]) add_outflow(a, dt, -F0[2], a.inv_dy);
             // M5, folded into the flux differences: -dt/dx (dF - S dx)
             const T Sx = T(0.5) * a.g * (hf[0] + hf[1]) * (zf[0] - zf[1]);
             const T Sy = T(0.5) * a.g * (hf[2] + hf[3]) * (zf[2] - zf[3]);

@@ -67,6 +67,8 @@ struct sim {
     uint8_t *chunk_flag = nullptr;
     void *ghost_zero = nullptr, *ghost_inf = nullptr;   // one strip-wide row each (TMA kernel, rows beyond the domain)
     int exit_i[16]{}, exit_j[16]{};
+    int door_cells[16]{}, door_target[16]{};
+    double *door_credit = nullptr;             // [16] device
     cudaGraphExec_t graph[GRAPH_LEVELS]{};          // graph[k] advances 2^k coupled steps; built on first use
     int device = 0;                   // the device the handle lives on; every entry point runs on it
     int n_sm = 148;
@@ -112,6 +114,7 @@ size_t layout(sim *s, Bump &b)
     const size_t rs = real_size(s), nc = (size_t)s->ncell, np = (size_t)s->np;
     auto real = [&](size_t n) { return (void *)b.take<char>(n * rs); };
     s->ctl = b.take<Ctl>(1);
+    s->door_credit = b.take<double>(16);
     s->stat_d = b.take<double>(8);
     s->stat_hist = b.take<unsigned long long>(8);
     for (int k = 0; k < 2; ++k) { s->h[k] = real(nc); s->qx[k] = real(nc); s->qy[k] = real(nc); }
@@ -219,6 +222,7 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     for (int k = 0; k < 4; ++k) a.inflow[k] = s->inflow[k];
     a.chunk_flag = s->chunk_flag; a.R = s->march_R;
     a.ghost_zero = (const T *)s->ghost_zero; a.ghost_inf = (const T *)s->ghost_inf; a.ghost_occ = (const uint8_t *)s->ghost_zero;
+    a.open_sides = s->prm.open_sides;
     a.ctl = s->ctl;
     return a;
 }
@@ -270,6 +274,12 @@ template <typename T> TailArgs<T> tail_args(const sim *s)
     a.layer_thickness = (T)s->prm.layer_thickness;
     a.hydro_t = s->hydro_t; a.hydro_q = s->hydro_q; a.n_hydro = s->n_hydro;
     a.inv_inflow_length = s->inflow_length > 0 ? 1.0 / s->inflow_length : 0.0;
+    a.A = ped_soa<T>(s, 0); a.np = s->np; a.n_doors = s->prm.n_doors; a.nx = s->grid.nx;
+    for (int d = 0; d < s->prm.n_doors; ++d) a.door_cells[d] = s->door_cells[d];
+    a.door_credit = s->door_credit;
+    a.spawn_rate = s->prm.spawn_rate; a.vpref_lo = s->prm.spawn_vpref_lo; a.vpref_hi = s->prm.spawn_vpref_hi;
+    a.dx = s->grid.dx; a.dy = s->grid.dy; a.target_population = s->prm.target_population;
+    a.seed_lo = (unsigned)(s->prm.spawn_seed & 0xffffffffull); a.seed_hi = (unsigned)(s->prm.spawn_seed >> 32);
     return a;
 }
 
@@ -280,6 +290,11 @@ template <typename T> PedArgs<T> ped_args_full(const sim *s, int pipelined)
     PedArgs<T> pa = ped_args<T>(s);
     for (int e = 0; e < s->prm.n_exit_cells; ++e) { pa.exit_i[e] = s->exit_i[e]; pa.exit_j[e] = s->exit_j[e]; }
     pa.n_exit = s->prm.n_exit_cells;
+    pa.n_doors = s->prm.n_doors;
+    for (int d = 0; d < s->prm.n_doors; ++d) {
+        pa.door_i[d] = s->door_cells[d] % s->grid.nx; pa.door_j[d] = s->door_cells[d] / s->grid.nx;
+        pa.door_target[d] = s->door_target[d];
+    }
     pa.pipelined = pipelined;
     pa.pdl_early = s->np >= 65536;   // measured: pre-scheduling the chain pays on Config 5 (-1.5 %), costs on Configs 1-3 (+8 %)
     return pa;
@@ -546,6 +561,7 @@ int upload_state(sim *s, const sim_topo_t *topo, const void *manning, const sim_
             upload(s, s->P[0].vpref, peds->v_pref, np * rs) || upload(s, s->P[0].role, peds->role, np))
             return SIM_ECUDA;
         std::vector<uint8_t> fsm(np), act(np, 1);
+        if (peds->active) for (size_t i = 0; i < np; ++i) act[i] = peds->active[i] ? 1 : 0;
         std::vector<int32_t> id(np), neg(np, -1);
         for (size_t i = 0; i < np; ++i) {
             fsm[i] = (peds->role && peds->role[i]) ? SIM_FSM_TO_STORAGE : SIM_FSM_EVACUATE;
@@ -597,6 +613,18 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         return bail(fail(s, SIM_EINVAL, "tau, B_s, g, cfl must be positive"));
     if (!(p->h_dry > 0) || (grid->real_bits == 32 && p->h_dry < 1.2e-38))
         return bail(fail(s, SIM_EINVAL, "h_dry must be positive (and a normal number in the storage precision): depths are divided by max(h, h_dry)"));
+    if (p->open_sides < 0 || p->open_sides > 15) return bail(fail(s, SIM_EINVAL, "open_sides is a mask of the four sides"));
+    if (p->n_doors < 0 || p->n_doors > 16) return bail(fail(s, SIM_EINVAL, "at most 16 doors"));
+    if (p->n_doors > 0) {
+        if (!p->door_cells || !p->door_target) return bail(fail(s, SIM_EINVAL, "door_cells and door_target are required when n_doors > 0"));
+        if (!(p->spawn_rate >= 0) || p->target_population < 0 || !(p->spawn_vpref_hi >= p->spawn_vpref_lo) || !(p->spawn_vpref_lo > 0))
+            return bail(fail(s, SIM_EINVAL, "spawn_rate, target_population >= 0 and 0 < spawn_vpref_lo <= spawn_vpref_hi are required"));
+        for (int d = 0; d < p->n_doors; ++d) {
+            const int c = p->door_cells[d];
+            if (c < 0 || c >= grid->nx * grid->ny || (topo->mask && topo->mask[c])) return bail(fail(s, SIM_EINVAL, "door cell out of range or solid"));
+            if (p->door_target[d] < 0 || p->door_target[d] >= p->n_targets) return bail(fail(s, SIM_EINVAL, "door target out of range"));
+        }
+    }
     if (p->flood_order < 0 || p->flood_order > 2) return bail(fail(s, SIM_EINVAL, "flood_order must be 0, 1 (first order, the paper's scheme) or 2 (MUSCL-Hancock)"));
     if (!(p->A_s > 0) || !(p->radius >= 0) || !(p->vmax_factor > 0))
         return bail(fail(s, SIM_EINVAL, "A_s and vmax_factor must be positive, radius non-negative"));
@@ -642,7 +670,11 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         s->prm.dt_max = grid->real_bits == 64 ? default_dt_max<double>(peds, p, dmin) : default_dt_max<float>(peds, p, dmin);
     }
     s->flood_variant = ((long long)nx * ny >= (1ll << 22)) ? (nx % 16 == 0 ? 4 : nx % 2 == 0 ? 3 : 2) : (nx % 4 == 0) ? 1 : 0;
+    if (p->open_sides) s->flood_variant = 0;       // open edges: the one-thread-per-cell kernel (and the MUSCL kernel)
     if (p->flood_order == 2) s->flood_variant = 5;
+    for (int d = 0; d < p->n_doors; ++d) { s->door_cells[d] = p->door_cells[d]; s->door_target[d] = p->door_target[d]; }
+    // doors: newcomers are placed by the tail kernel, so the binning of the next step must come after it
+    if (p->n_doors > 0) s->overlap = 0;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -754,8 +786,25 @@ extern "C" int sim_set_overlap(sim_t *s, int32_t on)
     if (!s) return SIM_EINVAL;
     DeviceGuard on_device(s);
     CU(cudaStreamSynchronize(s->stream));
+    if (on && s->prm.n_doors > 0) return fail(s, SIM_EINVAL, "with doors the step is one chain: newcomers are placed before the binning of the next step");
     s->overlap = on ? 1 : 0;
     drop_graphs(s);
+    return SIM_OK;
+}
+
+extern "C" int sim_test_philox(sim_t *s, const uint32_t *in, uint32_t *out, int32_t n)
+{
+    if (!s || !in || !out || n < 0) return SIM_EINVAL;
+    DeviceGuard on_device(s);
+    if (n == 0) return SIM_OK;
+    unsigned *d = nullptr;
+    CU(cudaMalloc(&d, (size_t)n * 10 * sizeof(unsigned)));
+    struct Free { unsigned *p; ~Free() { cudaFree(p); } } fr{d};
+    CU(cudaMemcpyAsync(d, in, (size_t)n * 6 * sizeof(unsigned), cudaMemcpyHostToDevice, s->stream));
+    philox_test_kernel<<<(n + 127) / 128, 128, 0, s->stream>>>(d, d + (size_t)n * 6, n);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out, d + (size_t)n * 6, (size_t)n * 4 * sizeof(unsigned), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     return SIM_OK;
 }
 
@@ -767,6 +816,7 @@ extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
     DeviceGuard on_device(s);
     if (variant < 0 || variant > 4) return fail(s, SIM_EINVAL, "variant must be 0..4");
     if (s->prm.flood_order == 2) return fail(s, SIM_EINVAL, "flood_order = 2 has one kernel (variant 5)");
+    if (s->prm.open_sides && variant != 0) return fail(s, SIM_EINVAL, "open edges are built into variants 0 and 5 only");
     if (variant == 4 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
     if (variant == 3 && s->grid.nx % 2 != 0) return fail(s, SIM_EINVAL, "the two-column march kernel needs nx % 2 == 0");
     if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");
@@ -842,6 +892,7 @@ template <typename T> int stats_t(sim *s, sim_stats_t *o)
     o->neg_depth_clamps = (int64_t)c.neg_clamps; o->clamped_volume = c.clamped_volume;
     o->cursor = c.cursor; o->layer = c.layer; o->bags = c.bags; o->barrier_complete = c.complete;
     o->deposits = c.deposits;
+    o->outflow_volume = c.outflow_volume; o->spawned = c.spawned; o->triggered = c.triggered;
     if (d[3] > 0 || d[4] > 0) return fail(s, SIM_ENOTFINITE, "non-finite depth, discharge or position");
     return SIM_OK;
 }

@@ -29,6 +29,7 @@ struct PedArgs {
     int n_targets, exit_target, storage_target, drop_target;
     int n_exit; int exit_i[16], exit_j[16];
     int storage_i, storage_j, drop_i, drop_j, arrive;
+    int n_doors; int door_i[16], door_j[16], door_target[16];   // entrance doors: fsm = FSM_WANDER + destination door
     PedSoA<T> A, B;                  // A: level n (any order) and level n+1; B: level n sorted by bin
     VecN<T, 2> *bxy;                 // (x, y) of B interleaved: one 64/128-bit load per candidate
     T c_exp1, c_exp2;                // fp32 pair force: A_s e^{(2r-d)/B_s} = 2^{c_exp1 + c_exp2 d}
@@ -47,6 +48,8 @@ struct PedArgs {
     const T *h[2], *qx[2], *qy[2];   // flood state (level n is [ctl->parity])
     Ctl *ctl;
 };
+
+constexpr int FSM_WANDER = 8;        // include/floodped.h SIM_FSM_WANDER
 
 // Which N_p buffer a kernel of the binning chain fills, or -1 if the chain must not run.
 // Pipelined (beside the tail kernel of the step before, which is rewriting parity and halt):
@@ -344,16 +347,21 @@ __device__ __forceinline__ void ped_step_one(const PedArgs<T> &a, const int d)
 #pragma unroll PED_UNROLL_K
         for (int j = s0; j < s1; ++j) pair_add(a, kc, x, y, a.bxy[j], ax, ay);
     }
+    // D7: once water is in the domain those still wandering become evacuees;
+    // D6: before that a wanderer leaves through its destination door, not through the exit
+    bool out = false;
+    if (fsm >= FSM_WANDER) {
+        if (a.ctl->triggered) fsm = 0;
+        else out = max(abs(ix - a.door_i[fsm - FSM_WANDER]), abs(iy - a.door_j[fsm - FSM_WANDER])) <= a.arrive;
+    }
     // 8. exit (C29): level-n cell within arrive_cells of an exit cell
-    if (role == 0 || fsm == 0) {
-        bool out = false;
+    if (fsm < FSM_WANDER && (role == 0 || fsm == 0))
         for (int e = 0; e < a.n_exit; ++e)
             out |= max(abs(ix - a.exit_i[e]), abs(iy - a.exit_j[e])) <= a.arrive;
-        if (out) {
-            A.x[d] = x; A.y[d] = y; A.vx[d] = vx; A.vy[d] = vy; A.timer[d] = timer;
-            A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 0;
-            return;
-        }
+    if (out) {
+        A.x[d] = x; A.y[d] = y; A.vx[d] = vx; A.vy[d] = vy; A.timer[d] = timer;
+        A.fsm[d] = fsm; A.state[d] = state; A.active[d] = 0;
+        return;
     }
     // 1. sample U^n at the containing cell -> HR -> Table 1 (C17-C20)
     const int p = a.ctl->parity;
@@ -372,6 +380,7 @@ __device__ __forceinline__ void ped_step_one(const PedArgs<T> &a, const int d)
     // 3. desired direction from the navigation field of the current target
     int target = a.exit_target;
     if (fsm == 1) target = a.storage_target; else if (fsm == 3) target = a.drop_target;
+    else if (fsm >= FSM_WANDER) target = a.door_target[fsm - FSM_WANDER];
     const int code = a.nav[(size_t)target * ((size_t)a.nx * a.ny) + c];
     T ex = T(0), ey = T(0);
     if (code < 8) {
@@ -447,7 +456,78 @@ struct TailArgs {
     const double *hydro_t, *hydro_q;
     int n_hydro;
     double inv_inflow_length;
+    // entrance doors
+    PedSoA<T> A;                     // level n+1 pedestrians (after the pedestrian step of this step)
+    int np, n_doors, nx;
+    int door_cells[16];
+    double *door_credit;             // [16] newcomers owed by each door
+    double spawn_rate, vpref_lo, vpref_hi, dx, dy;
+    int target_population;
+    unsigned int seed_lo, seed_hi;
 };
+
+// Philox4x32-10 (Salmon et al., SC'11) written from its definition; known answers: tests/test_boundary.py
+__device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0, unsigned k1, unsigned out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const unsigned h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+__global__ void philox_test_kernel(const unsigned *in /* [n][6] */, unsigned *out /* [n][4] */, int n)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) philox4x32_10(in[6 * k], in[6 * k + 1], in[6 * k + 2], in[6 * k + 3], in[6 * k + 4], in[6 * k + 5], out + 4 * k);
+}
+
+// D3-D5: the doors let newcomers in.  One warp; every lane holds the same copy of the control block.
+// The free-slot search (lowest original index among the inactive slots, D4) and the head count
+// are strided scans over the level n+1 arrays with a warp reduction: once per newcomer, which is a
+// few per step at most (10 per door).
+template <typename T>
+__device__ __forceinline__ void spawn_warp(const TailArgs<T> &a, long long &spawned, const double dt_taken)
+{
+    const int lane = threadIdx.x & 31;
+    const volatile uint8_t *act = a.A.active;
+    int pop = 0;
+    for (int s = lane; s < a.np; s += 32) pop += act[s] ? 1 : 0;
+    pop = __reduce_add_sync(0xffffffffu, pop);
+    for (int d = 0; d < a.n_doors; ++d) {
+        double cr = __dadd_rn(a.door_credit[d], __dmul_rn(a.spawn_rate, dt_taken));
+        while (cr >= 1.0) {
+            unsigned long long best = ~0ull;
+            if (pop < a.target_population)
+                for (int s = lane; s < a.np; s += 32)
+                    if (!act[s]) { const unsigned long long k = ((unsigned long long)(unsigned)a.A.id[s] << 32) | (unsigned)s; best = k < best ? k : best; }
+            for (int o = 16; o > 0; o >>= 1) { const unsigned long long t = __shfl_xor_sync(0xffffffffu, best, o); best = t < best ? t : best; }
+            if (best == ~0ull) { cr = 1.0; break; }                     // full: the door waits, owing one
+            if (lane == 0) {
+                const int s = (int)(unsigned)(best & 0xffffffffull);
+                unsigned r[4];
+                philox4x32_10((unsigned)(spawned & 0xffffffffll), (unsigned)(spawned >> 32), 0u, 0u, a.seed_lo, a.seed_hi, r);
+                const int dest = (int)(((unsigned long long)r[0] * (unsigned long long)a.n_doors) >> 32);
+                const double k32 = 1.0 / 4294967296.0;
+                const double ux = __dmul_rn((double)r[1], k32), uy = __dmul_rn((double)r[2], k32), uv = __dmul_rn((double)r[3], k32);
+                const int ci = a.door_cells[d] % a.nx, cj = a.door_cells[d] / a.nx;
+                a.A.x[s] = (T)__dmul_rn(__dadd_rn(__dadd_rn((double)ci, 0.1), __dmul_rn(0.8, ux)), a.dx);
+                a.A.y[s] = (T)__dmul_rn(__dadd_rn(__dadd_rn((double)cj, 0.1), __dmul_rn(0.8, uy)), a.dy);
+                a.A.vx[s] = T(0); a.A.vy[s] = T(0); a.A.timer[s] = T(0);
+                a.A.vpref[s] = (T)__dadd_rn(a.vpref_lo, __dmul_rn(__dadd_rn(a.vpref_hi, -a.vpref_lo), uv));
+                a.A.role[s] = 0; a.A.state[s] = 0; a.A.fsm[s] = (uint8_t)(FSM_WANDER + dest);
+                a.A.active[s] = 1;
+                __threadfence();
+            }
+            __syncwarp();
+            cr = __dadd_rn(cr, -1.0); spawned += 1; pop += 1;
+        }
+        if (lane == 0) a.door_credit[d] = cr;
+    }
+}
 
 __device__ __forceinline__ double hydrograph(const double *t, const double *q, int n, double time)
 {
@@ -516,6 +596,10 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
         l.parity ^= 1;
     }
     const double lam = __longlong_as_double((long long)l.lam_bits);
+    // D7, D8: a wet cell exists in U^{n+1} (its wave speed is positive) -> triggered, for good;
+    // D3: otherwise the doors let newcomers in (they exist from level n+1 on)
+    if (lam > 0.0) l.triggered = 1;
+    if (!first && !l.triggered && a.n_doors > 0) spawn_warp(a, l.spawned, l.dt);
     double dt = l.dt_max;
     if (lam > 0.0) dt = fmin(dt, l.cfl / lam);
     if (l.t + dt > l.t_end) dt = fmax(0.0, l.t_end - l.t);
@@ -523,6 +607,7 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
     if (threadIdx.x == 0) {
         if (!first) { c->D = 0; c->t = l.t; c->step = l.step; c->parity = l.parity; }
         c->dt = dt;
+        c->triggered = l.triggered; c->spawned = l.spawned;
         c->lam_bits = 0ull;
         c->halt = (l.t >= l.t_end) ? 1 : 0;
         c->q_in = q_in;

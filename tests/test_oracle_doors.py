@@ -12,8 +12,7 @@ import pytest
 
 import oracle
 from paper_1908_05232_b200 import scenarios as S
-from paper_1908_05232_b200.scenarios import nav_field
-from helpers import box, GOLDEN
+from helpers import box, GOLDEN, doors_box as _doors_box
 
 G = 9.81
 W, E, So, N = 1, 2, 4, 8
@@ -112,22 +111,6 @@ def test_inflow_faces_stay_inflow_on_an_open_side():
 
 
 # ------------------------------------------------------------------ D3, D4: doors
-
-def _doors_box(n=24, slots=64, rate=0.5, target=1000, n_doors=3, **kw):
-    """dry closed box, dt = dt_max = 0.25 s exactly, doors on the west wall, exit at the east wall"""
-    mask = np.zeros((n, n), np.uint8)
-    doors = np.array([(3 + 6 * d) * n + 0 for d in range(n_doors)], np.int32)
-    exit_cell = (n // 2) * n + n - 1
-    navs = [nav_field(mask, [exit_cell])[0]] + [nav_field(mask, [int(c)])[0] for c in doors]
-    sc = box(n, n, dx=1.0, h0=0.0, manning=0.0, dt_max=0.25,
-             peds=dict(x=np.full(slots, 12.5), y=np.full(slots, 12.5)), **kw)
-    sc.nav_dir = np.stack(navs); sc.exit_cells = np.array([exit_cell], np.int32); sc.exit_target = 0
-    sc.door_cells = doors; sc.door_target = np.arange(1, n_doors + 1, dtype=np.int32)
-    sc.spawn_rate = rate; sc.target_population = target; sc.spawn_seed = 1234
-    sc.spawn_vpref_lo, sc.spawn_vpref_hi = 1.0, 1.4
-    sc.pactive0 = np.zeros(slots, np.uint8)
-    return sc
-
 
 def test_spawn_cadence_closed_form():
     """rate 0.5 /s/door at dt = 0.25 s: the credit grows by exactly 1/8 a step, so every door lets one
