@@ -81,6 +81,12 @@ typedef struct {
     int32_t nx, ny;
     double  dx, dy;                             /* cell size, m                  */
     int32_t real_bits;                          /* 32 or 64                               */
+    /* Row slab (both 0 = the whole grid).  This handle holds the flood cells of rows
+     * [slab_j0, slab_j0 + ny) of a grid of slab_ny_global rows.  Every array given to sim_create
+     * (z, mask, h0, u0, v0, manning, nav_dir) is then the array of the WHOLE grid, every cell index
+     * (inflow, exit, door, barrier cells) is a cell of the whole grid, and the handle takes what it
+     * needs.  sim_read_* / sim_write_flood move the slab's rows only.  See sim_slab_link(). */
+    int32_t slab_j0, slab_ny_global;
 } sim_grid_t;
 
 typedef struct {                                /* flood agents' initial state    */
@@ -219,6 +225,25 @@ int sim_set_march_rows(sim_t *s, int32_t rows);
 int sim_set_overlap(sim_t *s, int32_t on);
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
+
+/* ---- row slabs across GPUs (SURVEY 8f-4, S:8e) ----
+ * The flood grid is cut into n <= 8 slabs of whole rows, one handle per slab, in row order, each on
+ * its own device (or, for testing, several on one device); all slabs but the last have the same
+ * number of rows.  sim_slab_link makes the handles one simulation:
+ *   - the flood kernel of a slab reads the one halo row it needs from the neighbour slab IN PLACE
+ *     (peer memory: the handles must be in one process with peer access, which this call enables;
+ *     no halo buffers, no exchange kernel); "immediate neighbours";
+ *   - the global time step is the minimum over the slabs: one 8-byte max-reduction of the wave
+ *     speed per step;
+ *   - all pedestrians live on handles[0] (the other handles are created with n = 0): its
+ *     pedestrian kernels sample depth and velocity of whichever slab holds the cell, write N_p
+ *     there and raise the bed there, again in place.
+ * Flood kernels: variant 4 (nx % 16 == 0) or 0.  Not combined with open edges or flood_order 2.
+ * sim_slab_step advances all slabs by n coupled steps (host-sequenced launches on the handles'
+ * streams, events between them; no kernel waits on another); sim_step on a linked handle fails.
+ * Results are bit-identical to the single-handle run of the whole grid. */
+int sim_slab_link(sim_t *const *handles, int32_t n);
+int sim_slab_step(sim_t *const *handles, int32_t n, int64_t steps);
 
 const char *sim_last_error(const sim_t *s);     /* s may be NULL: error of the last failed create */
 void sim_destroy(sim_t *s);

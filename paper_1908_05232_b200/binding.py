@@ -20,7 +20,7 @@ EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
     "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap",
-    "sim_kernels_per_step", "sim_last_error", "sim_destroy",
+    "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_last_error", "sim_destroy",
 ]
 
 _vp = C.c_void_p
@@ -31,7 +31,7 @@ _f64p = C.POINTER(C.c_double)
 
 class SimGrid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dx", C.c_double), ("dy", C.c_double),
-                ("real_bits", C.c_int32)]
+                ("real_bits", C.c_int32), ("slab_j0", C.c_int32), ("slab_ny_global", C.c_int32)]
 
 
 class SimTopo(C.Structure):
@@ -119,6 +119,8 @@ def load_library(path: str = LIB_PATH):
     L.sim_set_march_rows.argtypes = [_vp, C.c_int32]
     L.sim_set_overlap.argtypes = [_vp, C.c_int32]
     L.sim_kernels_per_step.argtypes = [_vp]
+    L.sim_slab_link.argtypes = [C.POINTER(_vp), C.c_int32]
+    L.sim_slab_step.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int64]
     L.sim_last_error.argtypes = [_vp]
     L.sim_last_error.restype = C.c_char_p
     L.sim_destroy.argtypes = [_vp]
@@ -137,7 +139,7 @@ def _np_ptr(a):
 class _Marshalled:
     """Host-side C structs for a Scenario; keeps the numpy arrays alive."""
 
-    def __init__(self, sc):
+    def __init__(self, sc, slab=None, with_peds=True):
         real = np.float64 if sc.real_bits == 64 else np.float32
         self.real = real
         self.keep = []
@@ -153,11 +155,14 @@ class _Marshalled:
             a = arr(a, dtype)
             return C.cast(None, ptype) if a is None or a.size == 0 else a.ctypes.data_as(ptype)
 
-        self.grid = SimGrid(sc.nx, sc.ny, sc.dx, sc.dy, sc.real_bits)
+        if slab is None:
+            self.grid = SimGrid(sc.nx, sc.ny, sc.dx, sc.dy, sc.real_bits, 0, 0)
+        else:                                       # rows [j0, j0 + ny_local) of the grid; arrays stay those of the whole grid
+            self.grid = SimGrid(sc.nx, slab[1], sc.dx, sc.dy, sc.real_bits, slab[0], sc.ny)
         self.topo = SimTopo(_np_ptr(arr(sc.z, real)), typed(sc.mask, np.uint8, _u8p),
                             _np_ptr(arr(sc.h0, real)), _np_ptr(arr(sc.u0, real)), _np_ptr(arr(sc.v0, real)))
         self.manning = arr(sc.manning, real)
-        n = int(sc.px.shape[0])
+        n = int(sc.px.shape[0]) if with_peds else 0
         self.peds = SimPeds(n, _np_ptr(arr(sc.px, real)), _np_ptr(arr(sc.py, real)),
                             _np_ptr(arr(sc.pvx, real)), _np_ptr(arr(sc.pvy, real)),
                             _np_ptr(arr(sc.pvpref, real)), typed(sc.prole, np.uint8, _u8p),
@@ -211,7 +216,7 @@ def workspace_bytes(sc) -> int:
 class Sim:
     """One simulation handle on the current CUDA device / current torch stream."""
 
-    def __init__(self, sc, device="cuda:0", use_torch_workspace=True, stream=None):
+    def __init__(self, sc, device="cuda:0", use_torch_workspace=True, stream=None, slab=None, with_peds=True):
         import torch
 
         L = load_library()
@@ -221,9 +226,10 @@ class Sim:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.real = np.float64 if sc.real_bits == 64 else np.float32
-        self.nx, self.ny, self.ncell, self.n_peds = sc.nx, sc.ny, sc.nx * sc.ny, int(sc.px.shape[0])
+        self.nx, self.ny = sc.nx, (sc.ny if slab is None else slab[1])
+        self.ncell, self.n_peds = self.nx * self.ny, (int(sc.px.shape[0]) if with_peds else 0)
         self.dx, self.dy = float(sc.dx), float(sc.dy)
-        m = _Marshalled(sc)
+        m = _Marshalled(sc, slab, with_peds)
         self._ws = None
         ws_ptr = None
         if use_torch_workspace:
@@ -349,3 +355,55 @@ class Sim:
 
     def set_barrier(self, cursor, layer, bags, complete):
         self._chk(self._L.sim_set_barrier(self._h, int(cursor), int(layer), int(bags), int(complete)))
+
+
+class SlabSim:
+    """The grid cut into `n_slabs` row slabs, one handle each (include/floodped.h
+    sim_slab_link): `devices` names one CUDA device per slab (all in this process, with peer access),
+    default all on `cuda:0`, which is how the path is tested on one GPU.  All pedestrians live on
+    the first slab's handle.  Marshalling only."""
+
+    def __init__(self, sc, n_slabs, devices=None):
+        from .replicas import slab_cuts
+        self.cuts = slab_cuts(sc.ny, n_slabs)
+        devices = devices or ["cuda:0"] * len(self.cuts)
+        self.sims = [Sim(sc, device=devices[r], slab=cut, with_peds=(r == 0)) for r, cut in enumerate(self.cuts)]
+        self._L = self.sims[0]._L
+        self._arr = (_vp * len(self.sims))(*[g._h for g in self.sims])
+        self._chk(self._L.sim_slab_link(self._arr, len(self.sims)))
+
+    def _chk(self, rc):
+        if rc != SIM_OK:
+            raise FloodpedError(rc, self._L.sim_last_error(self.sims[0]._h).decode())
+
+    def step(self, n=1):
+        self._chk(self._L.sim_slab_step(self._arr, len(self.sims), int(n)))
+
+    def read_conserved(self):
+        parts = [g.read_conserved() for g in self.sims]
+        return {k: np.concatenate([p[k] for p in parts]) for k in ("h", "qx", "qy")}
+
+    def read_flood(self, fields=("h", "u", "v", "z", "hr")):
+        parts = [g.read_flood(fields) for g in self.sims]
+        return {k: np.concatenate([p[k] for p in parts]) for k in fields}
+
+    def read_occupancy(self):
+        return np.concatenate([g.read_occupancy() for g in self.sims])
+
+    def read_peds(self):
+        return self.sims[0].read_peds()
+
+    def stats(self) -> dict:
+        """the first slab's record (time, pedestrians, barrier) with the flood sums taken over all slabs"""
+        st = [g.stats() for g in self.sims]
+        d = dict(st[0])
+        d["volume"] = float(sum(s["volume"] for s in st))
+        d["clamped_volume"] = float(sum(s["clamped_volume"] for s in st))
+        d["neg_depth_clamps"] = int(sum(s["neg_depth_clamps"] for s in st))
+        d["max_h"] = max(s["max_h"] for s in st); d["max_hr"] = max(s["max_hr"] for s in st)
+        d["per_slab"] = st
+        return d
+
+    def close(self):
+        for g in self.sims:
+            g.close()

@@ -35,6 +35,11 @@ struct FloodArgs {
     const T *ghost_zero, *ghost_inf;  // one strip-wide row of zeros / of +inf, and of zero bytes: the row beyond the
     const uint8_t *ghost_occ;         // domain edge as the TMA kernel loads it (a wall = a row of solid cells, C13)
     int R;                            // march kernel: rows per chunk
+    // row slabs: the row below my first row / above my last row is the boundary row of the
+    // neighbour slab, read in place -- peer memory over NVLink, or another handle on the same device.
+    // [0 south | 1 north][flood parity]; null = the domain edge (wall ghost).  Kernels 0 and 4.
+    const T *halo_h[2][2], *halo_qx[2][2], *halo_qy[2][2];
+    const T *halo_z[2];
     int open_sides;                   // bit per domain edge (W, E, S, N): open, transmissive ghost; kernels 0 and 5 only
     Ctl *ctl;
 };
@@ -184,6 +189,10 @@ __global__ void __launch_bounds__(256) flood_cell_kernel(FloodArgs<T> a)
                     const int k = jj * a.nx + ii;
                     zk = Z[k];
                     if (!is_solid(zk)) { hk = H[k]; primitives(hk, QX[k], QY[k], a.h_dry, uk, vk); }
+                } else if ((jj < 0 || jj >= a.ny) && ii >= 0 && ii < a.nx && a.halo_z[jj < 0 ? 0 : 1]) {
+                    const int sd = jj < 0 ? 0 : 1;                          // the neighbour slab's boundary row (8f-4)
+                    zk = a.halo_z[sd][ii];
+                    if (!is_solid(zk)) { hk = a.halo_h[sd][p][ii]; primitives(hk, a.halo_qx[sd][p][ii], a.halo_qy[sd][p][ii], a.h_dry, uk, vk); }
                 } else if (open) { hk = h; uk = u; vk = v; zk = z; }       // transmissive ghost (D1)
             };
             T hk, uk, vk, zk, f1L, f1R;

@@ -88,6 +88,16 @@ __device__ __forceinline__ void tm_issue_row(const FloodArgs<T> &a, const T *H, 
     constexpr uint32_t RB = MW * sizeof(T);
     mbar_expect_tx(bar, 5 * RB + MW);
     if (EDGE && (j < 0 || j >= a.ny)) {
+        const int sd = j < 0 ? 0 : 1, p = H == a.h[1] ? 1 : 0;
+        if (a.halo_z[sd]) {                            // row slab (8f-4): the neighbour slab's boundary row, read in place
+            bulk_g2s(st.h, a.halo_h[sd][p] + x0, RB, bar);
+            bulk_g2s(st.qx, a.halo_qx[sd][p] + x0, RB, bar);
+            bulk_g2s(st.qy, a.halo_qy[sd][p] + x0, RB, bar);
+            bulk_g2s(st.z, a.halo_z[sd] + x0, RB, bar);
+            bulk_g2s(st.n0, a.ghost_zero, RB, bar);
+            bulk_g2s(st.occ, a.ghost_occ, MW, bar);
+            return;
+        }
         bulk_g2s(st.h, a.ghost_zero, RB, bar);
         bulk_g2s(st.qx, a.ghost_zero, RB, bar);
         bulk_g2s(st.qy, a.ghost_zero, RB, bar);

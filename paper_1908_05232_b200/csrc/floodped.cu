@@ -43,6 +43,11 @@ struct sim {
     sim_grid_t grid{};
     sim_params_t prm{};             // scalar copy; pointers inside are NOT valid after create
     int ncell = 0, np = 0, kbin = 1, nbx = 0, nby = 0, nbins = 0;
+    // row slab: the flood arrays hold rows [j0, j0 + grid.ny) of a grid of gny rows; the
+    // pedestrians (all of them live on the first slab's handle) walk on the whole grid of pcell cells
+    int gny = 0, j0 = 0, pcell = 0;
+    sim *group[8]{}; int ngroup = 0, grank = 0;   // linked slabs in row order (sim_slab_link)
+    cudaEvent_t ev_slab = nullptr;
     int n_inflow = 0, n_hydro = 0, n_line = 0, n_targets = 0;
     double inflow_length = 0.0;
     cudaStream_t stream = nullptr, cap_stream = nullptr;
@@ -120,10 +125,10 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 2; ++k) { s->h[k] = real(nc); s->qx[k] = real(nc); s->qy[k] = real(nc); }
     s->zs = real(nc); s->z0 = real(nc); s->n0 = real(nc);
     for (int k = 0; k < 3; ++k) s->scratch_real[k] = real(nc);
-    s->occ = b.take<uint8_t>(2 * nc); s->mask = b.take<uint8_t>(nc);
+    s->occ = b.take<uint8_t>(2 * nc); s->mask = b.take<uint8_t>((size_t)(s->np > 0 ? s->pcell : 1));
     s->inflow[0] = b.take<uint8_t>(s->grid.ny); s->inflow[1] = b.take<uint8_t>(s->grid.ny);
     s->inflow[2] = b.take<uint8_t>(s->grid.nx); s->inflow[3] = b.take<uint8_t>(s->grid.nx);
-    s->nav = b.take<uint8_t>((size_t)s->n_targets * nc);
+    s->nav = b.take<uint8_t>(s->np > 0 ? (size_t)s->n_targets * s->pcell : 1);
     s->line_cells = b.take<int32_t>(s->n_line + 1);
     s->hydro_t = b.take<double>(s->n_hydro + 1); s->hydro_q = b.take<double>(s->n_hydro + 1);
     for (int k = 0; k < 2; ++k) {
@@ -164,9 +169,14 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
         }
     }
     s->ncell = g->nx * g->ny; s->np = n_peds;
+    s->gny = g->slab_ny_global > 0 ? g->slab_ny_global : g->ny;
+    s->j0 = g->slab_ny_global > 0 ? g->slab_j0 : 0;
+    if (s->j0 < 0 || s->j0 + g->ny > s->gny || (long long)g->nx * s->gny > 0x7fffffffLL)
+        return fail(s, SIM_EINVAL, "slab rows [slab_j0, slab_j0 + ny) must lie inside slab_ny_global rows");
+    s->pcell = g->nx * s->gny;
     const double dmin = g->dx < g->dy ? g->dx : g->dy;
     s->kbin = (int)std::ceil(p->R_int / dmin); if (s->kbin < 1) s->kbin = 1;     // C26
-    s->nbx = (g->nx + s->kbin - 1) / s->kbin; s->nby = (g->ny + s->kbin - 1) / s->kbin;
+    s->nbx = (g->nx + s->kbin - 1) / s->kbin; s->nby = (s->gny + s->kbin - 1) / s->kbin;
     s->nbins = s->nbx * s->nby;
     // march kernel geometry: strips of MW columns, chunks of R rows; R shrinks until the grid
     // fills the 148 SMs a few times over
@@ -223,6 +233,19 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     a.chunk_flag = s->chunk_flag; a.R = s->march_R;
     a.ghost_zero = (const T *)s->ghost_zero; a.ghost_inf = (const T *)s->ghost_inf; a.ghost_occ = (const uint8_t *)s->ghost_zero;
     a.open_sides = s->prm.open_sides;
+    if (s->ngroup > 1) {
+        const size_t nx = (size_t)s->grid.nx;
+        const sim *lo = s->grank > 0 ? s->group[s->grank - 1] : nullptr, *hi = s->grank + 1 < s->ngroup ? s->group[s->grank + 1] : nullptr;
+        if (lo) {
+            const size_t off = (size_t)(lo->grid.ny - 1) * nx;            // its last row
+            for (int k = 0; k < 2; ++k) { a.halo_h[0][k] = (const T *)lo->h[k] + off; a.halo_qx[0][k] = (const T *)lo->qx[k] + off; a.halo_qy[0][k] = (const T *)lo->qy[k] + off; }
+            a.halo_z[0] = (const T *)lo->zs + off;
+        }
+        if (hi) {                                                          // its first row
+            for (int k = 0; k < 2; ++k) { a.halo_h[1][k] = (const T *)hi->h[k]; a.halo_qx[1][k] = (const T *)hi->qx[k]; a.halo_qy[1][k] = (const T *)hi->qy[k]; }
+            a.halo_z[1] = (const T *)hi->zs;
+        }
+    }
     a.ctl = s->ctl;
     return a;
 }
@@ -241,7 +264,7 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
 {
     PedArgs<T> a{};
     const sim_params_t &p = s->prm;
-    a.n = s->np; a.nx = s->grid.nx; a.ny = s->grid.ny;
+    a.n = s->np; a.nx = s->grid.nx; a.ny = s->gny;
     a.kbin = s->kbin; a.nbx = s->nbx; a.nby = s->nby; a.nbins = s->nbins;
     a.inv_dx = (T)(1.0 / s->grid.dx); a.inv_dy = (T)(1.0 / s->grid.dy);
     a.h_dry = (T)p.h_dry;
@@ -256,12 +279,22 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
     a.arrive = p.arrive_cells;
     a.A = ped_soa<T>(s, 0); a.B = ped_soa<T>(s, 1);
     a.key = s->key; a.off = s->off; a.count = s->count; a.start = s->start; a.cellprev = s->cellprev;
-    a.occ = s->occ; a.mask = s->mask; a.nav = s->nav;
-    a.occ_stride = (size_t)s->ncell; a.cellprev_stride = (size_t)s->np; a.pipelined = 0;
+    a.mask = s->mask; a.nav = s->nav;
+    a.cellprev_stride = (size_t)s->np; a.pipelined = 0;
     a.bxy = (VecN<T, 2> *)s->bxy;
     a.c_exp1 = (T)(2.0 * p.radius / p.B_s * 1.4426950408889634 + std::log2(p.A_s));   // A e^{(2r-d)/B} = 2^{c1 + c2 d}
     a.c_exp2 = (T)(-1.4426950408889634 / p.B_s);
-    for (int k = 0; k < 2; ++k) { a.h[k] = (const T *)s->h[k]; a.qx[k] = (const T *)s->qx[k]; a.qy[k] = (const T *)s->qy[k]; }
+    // where the flood state of a cell lives: one slab (this handle's own grid) unless linked (8f-4)
+    const int ng = s->ngroup > 0 ? s->ngroup : 1;
+    a.slab.n = ng; a.slab.rows = ng > 1 ? s->group[0]->grid.ny : s->gny;
+    for (int r = 0; r < ng; ++r) {
+        const sim *q = ng > 1 ? s->group[r] : s;
+        const ptrdiff_t off = (ptrdiff_t)q->j0 * s->grid.nx;
+        for (int k = 0; k < 2; ++k) {
+            a.slab.h[k][r] = (const T *)q->h[k] - off; a.slab.qx[k][r] = (const T *)q->qx[k] - off; a.slab.qy[k][r] = (const T *)q->qy[k] - off;
+            a.slab.occ[k][r] = q->occ + (size_t)k * q->ncell - off;
+        }
+    }
     a.ctl = s->ctl;
     return a;
 }
@@ -269,12 +302,17 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
 template <typename T> TailArgs<T> tail_args(const sim *s)
 {
     TailArgs<T> a{};
-    a.ctl = s->ctl; a.zs = (T *)s->zs; a.line_cells = s->line_cells;
+    a.ctl = s->ctl; a.line_cells = s->line_cells;
+    {
+        const int ng = s->ngroup > 0 ? s->ngroup : 1;
+        a.slab_rows = ng > 1 ? s->group[0]->grid.ny : s->gny; a.nx = s->grid.nx;
+        for (int r = 0; r < ng; ++r) { const sim *q = ng > 1 ? s->group[r] : s; a.zs_tab[r] = (T *)q->zs - (ptrdiff_t)q->j0 * s->grid.nx; }
+    }
     a.n_line = s->n_line; a.bags_per_cell_layer = s->prm.bags_per_cell_layer; a.n_layers = s->prm.n_layers;
     a.layer_thickness = (T)s->prm.layer_thickness;
     a.hydro_t = s->hydro_t; a.hydro_q = s->hydro_q; a.n_hydro = s->n_hydro;
     a.inv_inflow_length = s->inflow_length > 0 ? 1.0 / s->inflow_length : 0.0;
-    a.A = ped_soa<T>(s, 0); a.np = s->np; a.n_doors = s->prm.n_doors; a.nx = s->grid.nx;
+    a.A = ped_soa<T>(s, 0); a.np = s->np; a.n_doors = s->prm.n_doors;
     for (int d = 0; d < s->prm.n_doors; ++d) a.door_cells[d] = s->door_cells[d];
     a.door_credit = s->door_credit;
     a.spawn_rate = s->prm.spawn_rate; a.vpref_lo = s->prm.spawn_vpref_lo; a.vpref_hi = s->prm.spawn_vpref_hi;
@@ -527,6 +565,14 @@ template <typename T>
 int upload_state(sim *s, const sim_topo_t *topo, const void *manning, const sim_peds_t *peds, const sim_params_t *p)
 {
     const size_t nc = (size_t)s->ncell, rs = sizeof(T);
+    // a row slab (8f-4) is given the arrays of the WHOLE grid and takes its rows of the flood fields
+    const size_t so = (size_t)s->j0 * s->grid.nx;
+    sim_topo_t cut = *topo;
+    cut.z = (const T *)topo->z + so; cut.mask = topo->mask ? topo->mask + so : nullptr;
+    cut.h0 = topo->h0 ? (const T *)topo->h0 + so : nullptr; cut.u0 = topo->u0 ? (const T *)topo->u0 + so : nullptr;
+    cut.v0 = topo->v0 ? (const T *)topo->v0 + so : nullptr;
+    const uint8_t *mask_all = topo->mask;
+    topo = &cut; manning = (const T *)manning + so;
     std::vector<T> tmp;
     make_zs<T>((const T *)topo->z, topo->mask, nc, tmp);
     if (upload(s, s->zs, tmp.data(), nc * rs)) return SIM_ECUDA;
@@ -538,7 +584,7 @@ int upload_state(sim *s, const sim_topo_t *topo, const void *manning, const sim_
     }
     if (upload(s, s->z0, topo->z, nc * rs)) return SIM_ECUDA;
     if (upload(s, s->n0, manning, nc * rs)) return SIM_ECUDA;
-    if (upload(s, s->mask, topo->mask, nc)) return SIM_ECUDA;
+    if (s->np > 0 && upload(s, s->mask, mask_all, (size_t)s->pcell)) return SIM_ECUDA;      // the pedestrians' mask: whole grid
     // depth: zero inside solids
     if (topo->h0) {
         tmp.resize(nc);
@@ -606,7 +652,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     if (!topo || !topo->z || !manning) return bail(fail(s, SIM_EINVAL, "z and manning are required"));
     if (n_peds > 0 && (!peds->x || !peds->y || !peds->vx || !peds->vy || !peds->v_pref))
         return bail(fail(s, SIM_EINVAL, "pedestrian arrays are required when n > 0"));
-    if (!p->nav_dir) return bail(fail(s, SIM_EINVAL, "nav_dir is required"));
+    if (n_peds > 0 && !p->nav_dir) return bail(fail(s, SIM_EINVAL, "nav_dir is required"));
     if (p->n_cap < 0 || p->n_cap > 255) return bail(fail(s, SIM_EINVAL, "n_cap must be in [0, 255]"));
     if (p->n_exit_cells > 16) return bail(fail(s, SIM_EINVAL, "at most 16 exit cells"));
     if (!(p->tau > 0) || !(p->B_s > 0) || !(p->g > 0) || !(p->cfl > 0))
@@ -621,7 +667,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
             return bail(fail(s, SIM_EINVAL, "spawn_rate, target_population >= 0 and 0 < spawn_vpref_lo <= spawn_vpref_hi are required"));
         for (int d = 0; d < p->n_doors; ++d) {
             const int c = p->door_cells[d];
-            if (c < 0 || c >= grid->nx * grid->ny || (topo->mask && topo->mask[c])) return bail(fail(s, SIM_EINVAL, "door cell out of range or solid"));
+            if (c < 0 || c >= s->pcell || (topo->mask && topo->mask[c])) return bail(fail(s, SIM_EINVAL, "door cell out of range or solid"));
             if (p->door_target[d] < 0 || p->door_target[d] >= p->n_targets) return bail(fail(s, SIM_EINVAL, "door target out of range"));
         }
     }
@@ -633,8 +679,8 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     if (p->exit_target < 0 || p->exit_target >= p->n_targets || p->storage_target < 0 ||
         p->storage_target >= p->n_targets || p->drop_target < 0 || p->drop_target >= p->n_targets)
         return bail(fail(s, SIM_EINVAL, "target index out of range"));
-    const int nx = grid->nx, ny = grid->ny;
-    auto cell_ok = [&](int c) { return c >= 0 && c < nx * ny; };
+    const int nx = grid->nx, ny = grid->ny, gny = s->gny, j0 = s->j0;      // cell indices are those of the whole grid
+    auto cell_ok = [&](int c) { return c >= 0 && c < nx * gny; };
     for (int e = 0; e < p->n_exit_cells; ++e)
         if (!cell_ok(p->exit_cells[e])) return bail(fail(s, SIM_EINVAL, "exit cell out of range"));
     if (!cell_ok(p->storage_cell) || !cell_ok(p->drop_cell)) return bail(fail(s, SIM_EINVAL, "storage/drop cell out of range"));
@@ -652,13 +698,14 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         if (!cell_ok(c) || side > 3) return bail(fail(s, SIM_EINVAL, "inflow face out of range"));
         const int i = c % nx, j = c / nx;
         const bool on_edge = (side == SIM_SIDE_W && i == 0) || (side == SIM_SIDE_E && i == nx - 1) ||
-                             (side == SIM_SIDE_S && j == 0) || (side == SIM_SIDE_N && j == ny - 1);
+                             (side == SIM_SIDE_S && j == 0) || (side == SIM_SIDE_N && j == gny - 1);
         if (!on_edge) return bail(fail(s, SIM_EINVAL, "inflow faces must lie on the domain edge (C14)"));
         if (topo->mask && topo->mask[c]) return bail(fail(s, SIM_EINVAL, "inflow face on a solid cell: its share of Q(t) would be lost"));
-        uint8_t &m = infl[side][side < 2 ? j : i];
+        s->inflow_length += side < 2 ? grid->dy : grid->dx;                 // of the whole grid: q_in = Q / length
+        if (j < j0 || j >= j0 + ny) continue;                                // another slab's face
+        uint8_t &m = infl[side][side < 2 ? j - j0 : i];
         if (m == 255) return bail(fail(s, SIM_EINVAL, "too many inflow faces on one cell side"));
         m += 1;
-        s->inflow_length += side < 2 ? grid->dy : grid->dx;
     }
     for (int k = 1; k < p->n_hydro; ++k)
         if (!(p->hydro_t[k] > p->hydro_t[k - 1])) return bail(fail(s, SIM_EINVAL, "hydro_t must increase"));
@@ -700,7 +747,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
         int r = DISPATCH(s, upload_state, s, topo, manning, peds, p);
         if (r != SIM_OK) return r;
         for (int k = 0; k < 4; ++k) if (upload(s, s->inflow[k], infl[k].data(), infl[k].size())) return SIM_ECUDA;
-        if (upload(s, s->nav, p->nav_dir, (size_t)p->n_targets * s->ncell)) return SIM_ECUDA;
+        if (s->np > 0 && upload(s, s->nav, p->nav_dir, (size_t)p->n_targets * s->pcell)) return SIM_ECUDA;
         if (p->n_line && upload(s, s->line_cells, p->line_cells, (size_t)p->n_line * 4)) return SIM_ECUDA;
         if (p->n_hydro && (upload(s, s->hydro_t, p->hydro_t, (size_t)p->n_hydro * 8) ||
                            upload(s, s->hydro_q, p->hydro_q, (size_t)p->n_hydro * 8))) return SIM_ECUDA;
@@ -730,6 +777,7 @@ extern "C" int sim_step(sim_t *s, int64_t n)
     if (!s) return SIM_EINVAL;
     DeviceGuard on_device(s);
     if (n < 0) return fail(s, SIM_EINVAL, "negative step count");
+    if (s->ngroup > 1) return fail(s, SIM_EINVAL, "a linked row slab steps with sim_slab_step");
     if (n == 0) return SIM_OK;
     {
         int rc = DISPATCH(s, prepare_bins, s);
@@ -790,6 +838,140 @@ extern "C" int sim_set_overlap(sim_t *s, int32_t on)
     s->overlap = on ? 1 : 0;
     drop_graphs(s);
     return SIM_OK;
+}
+
+// ---- row slabs
+namespace {
+
+template <typename T> int slab_refresh(sim *const *h, int n)
+{
+    SlabCtls t{}; t.n = n;
+    for (int r = 0; r < n; ++r) {
+        sim *s = h[r];
+        DeviceGuard g(s);
+        t.c[r] = s->ctl;
+        flood_chunk_flags_kernel<T><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const T *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
+        flood_lambda_kernel<T><<<592, 256, 0, s->stream>>>(flood_args<T>(s));
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(s->stream));
+    }
+    {
+        sim *s = h[0];
+        DeviceGuard g(s);
+        slab_lambda_kernel<<<1, 32, 0, s->stream>>>(t);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(s->stream));
+    }
+    for (int r = 0; r < n; ++r) {
+        sim *s = h[r];
+        DeviceGuard g(s);
+        tail_kernel<T><<<1, 32, 0, s->stream>>>(tail_args<T>(s), 1);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(s->stream));
+    }
+    return SIM_OK;
+}
+
+template <typename T> int slab_step(sim *const *h, int n, int64_t steps)
+{
+    sim *s0 = h[0];
+    SlabCtls t{}; t.n = n;
+    for (int r = 0; r < n; ++r) t.c[r] = h[r]->ctl;
+    {
+        sim *s = s0;
+        DeviceGuard g(s);
+        int rc = prepare_bins<T>(s);
+        if (rc != SIM_OK) return rc;
+    }
+    Marks none{nullptr, 0, s0->stream};
+    for (int64_t k = 0; k < steps; ++k) {
+        // fork: the other slabs start after everything of the step before (the binning chain wrote their N_p)
+        { sim *s = s0; DeviceGuard g(s); CU(cudaEventRecord(s0->ev_fork, s0->stream)); }
+        for (int r = 1; r < n; ++r) { sim *s = h[r]; DeviceGuard g(s); CU(cudaStreamWaitEvent(s->stream, s0->ev_fork, 0)); }
+        // pedestrian step (all pedestrians, on the first slab's device) and the flood kernels, all at level n
+        {
+            sim *s = s0; DeviceGuard g(s);
+            if (s->np > 0)
+                CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + PED_THREADS - 1) / PED_THREADS), dim3(PED_THREADS), 0, s->stream, false, ped_args_full<T>(s, 0), 0));
+        }
+        for (int r = 0; r < n; ++r) {
+            sim *s = h[r]; DeviceGuard g(s);
+            int rc = launch_flood<T>(s, s->stream, false);
+            if (rc != SIM_OK) return rc;
+            if (r) { CU(cudaEventRecord(s->ev_slab, s->stream)); CU(cudaStreamWaitEvent(s0->stream, s->ev_slab, 0)); }
+        }
+        // the global wave speed, then every slab's tail
+        { sim *s = s0; DeviceGuard g(s); slab_lambda_kernel<<<1, 32, 0, s->stream>>>(t); CU(cudaGetLastError()); CU(cudaEventRecord(s0->ev_ped, s0->stream)); }
+        for (int r = 0; r < n; ++r) {
+            sim *s = h[r]; DeviceGuard g(s);
+            if (r) CU(cudaStreamWaitEvent(s->stream, s0->ev_ped, 0));
+            CU(launch_pdl(tail_kernel<T>, dim3(1), dim3(32), 0, s->stream, false, tail_args<T>(s), 0));
+            if (r) { CU(cudaEventRecord(s->ev_slab, s->stream)); CU(cudaStreamWaitEvent(s0->stream, s->ev_slab, 0)); }
+        }
+        // binning chain of the next step (N_p goes to the slab that holds the cell)
+        {
+            sim *s = s0; DeviceGuard g(s);
+            if (s->np > 0) { int rc = enqueue_bin_chain<T>(s, s->stream, 0, none); if (rc != SIM_OK) return rc; }
+        }
+    }
+    return SIM_OK;
+}
+
+}  // namespace
+
+extern "C" int sim_slab_link(sim_t *const *h, int32_t n)
+{
+    if (!h || n < 1 || n > MAX_SLABS) return fail(nullptr, SIM_EINVAL, "1..8 slab handles");
+    sim *s = h[0];
+    if (!s) return SIM_EINVAL;
+    int row = 0;
+    for (int r = 0; r < n; ++r) {
+        sim *q = h[r];
+        if (!q) return fail(s, SIM_EINVAL, "null slab handle");
+        if (q->grid.nx != s->grid.nx || q->gny != s->gny || q->grid.real_bits != s->grid.real_bits || q->grid.dx != s->grid.dx || q->grid.dy != s->grid.dy)
+            return fail(s, SIM_EINVAL, "slabs must cut one grid");
+        if (q->j0 != row) return fail(s, SIM_EINVAL, "slabs must be given in row order and cover the grid without gaps");
+        if (r + 1 < n && q->grid.ny != s->grid.ny) return fail(s, SIM_EINVAL, "all slabs but the last must have the same number of rows");
+        if (r > 0 && q->np > 0) return fail(s, SIM_EINVAL, "all pedestrians live on the first slab's handle");
+        if (q->prm.open_sides || q->prm.flood_order == 2) return fail(s, SIM_EINVAL, "row slabs are not combined with open edges or flood_order 2");
+        if (q->ngroup) return fail(s, SIM_EINVAL, "handle is already linked");
+        row += q->grid.ny;
+    }
+    if (row != s->gny) return fail(s, SIM_EINVAL, "slabs must cover the grid");
+    // peer access between the devices of the slabs (one process)
+    for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b) {
+            if (h[a]->device == h[b]->device) continue;
+            int can = 0;
+            DeviceGuard g(h[a]);
+            if (cudaDeviceCanAccessPeer(&can, h[a]->device, h[b]->device) != cudaSuccess || !can)
+                return fail(s, SIM_ECUDA, "the devices of the slabs have no peer access");
+            cudaError_t e = cudaDeviceEnablePeerAccess(h[b]->device, 0);
+            if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return fail(s, SIM_ECUDA, cudaGetErrorString(e));
+            cudaGetLastError();
+        }
+    for (int r = 0; r < n; ++r) {
+        sim *q = h[r];
+        DeviceGuard g(q);
+        CU(cudaStreamSynchronize(q->stream));
+        drop_graphs(q);
+        q->ngroup = n; q->grank = r;
+        for (int k = 0; k < n; ++k) q->group[k] = h[k];
+        if (q->flood_variant != 0 && q->flood_variant != 4) q->flood_variant = q->grid.nx % 16 == 0 ? 4 : 0;
+        if (!q->ev_slab) CU(cudaEventCreateWithFlags(&q->ev_slab, cudaEventDisableTiming));
+        q->binned = false;
+    }
+    return s->grid.real_bits == 64 ? slab_refresh<double>(h, n) : slab_refresh<float>(h, n);
+}
+
+extern "C" int sim_slab_step(sim_t *const *h, int32_t n, int64_t steps)
+{
+    if (!h || n < 1 || !h[0]) return SIM_EINVAL;
+    sim *s = h[0];
+    if (s->ngroup != n) return fail(s, SIM_EINVAL, "sim_slab_link these handles first");
+    for (int r = 0; r < n; ++r) if (h[r] != s->group[r]) return fail(s, SIM_EINVAL, "not the linked handles, or not in their order");
+    if (steps < 0) return fail(s, SIM_EINVAL, "negative step count");
+    return s->grid.real_bits == 64 ? slab_step<double>(h, n, steps) : slab_step<float>(h, n, steps);
 }
 
 extern "C" int sim_test_philox(sim_t *s, const uint32_t *in, uint32_t *out, int32_t n)
@@ -859,7 +1041,7 @@ template <typename T> int read_peds_t(sim *s, void *x, void *y, void *vx, void *
     const int np = s->np;
     if (!np) return SIM_OK;
     ped_gather_kernel<T><<<(np + 255) / 256, 256, 0, s->stream>>>(
-        ped_soa<T>(s, 0), np, s->grid.nx, (T)(1.0 / s->grid.dx), (T)(1.0 / s->grid.dy), s->grid.ny,
+        ped_soa<T>(s, 0), np, s->grid.nx, (T)(1.0 / s->grid.dx), (T)(1.0 / s->grid.dy), s->gny,
         (T *)s->ped_out[0], (T *)s->ped_out[1], (T *)s->ped_out[2], (T *)s->ped_out[3],
         s->ped_out_u8[0], s->ped_out_u8[1], s->ped_out_u8[2], s->ped_out_i32[0], (T *)s->ped_out[4], nullptr);
     CU(cudaGetLastError());
@@ -912,7 +1094,7 @@ template <typename T> int bin_peds_t(sim *s, int32_t *key, int32_t *order, int32
         scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl, 0, 0);
         ped_scatter_kernel<T><<<nb, 256, 0, s->stream>>>(pa);
         ped_key_by_id_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 0), s->key, np, s->ped_out_i32[0]);
-        ped_gather_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 1), np, s->grid.nx, (T)1, (T)1, s->grid.ny,
+        ped_gather_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 1), np, s->grid.nx, (T)1, (T)1, s->gny,
             nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, s->ped_out_i32[1]);
         CU(cudaGetLastError());
         // (the scatter kernel has re-armed the scan)
@@ -1121,6 +1303,7 @@ extern "C" void sim_destroy(sim_t *s)
     if (s->ev_ped) cudaEventDestroy(s->ev_ped);
     if (s->ev_occ) cudaEventDestroy(s->ev_occ);
     if (s->ev_tail) cudaEventDestroy(s->ev_tail);
+    if (s->ev_slab) cudaEventDestroy(s->ev_slab);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
 }

@@ -19,6 +19,19 @@ struct PedSoA {
     int32_t *cell;                   // level-n containing cell (valid in the sorted buffer)
 };
 
+// Where the flood state of a cell lives: row slab r = row / rows holds the rows
+// [r rows, (r + 1) rows); every pointer is pre-offset so that it is indexed with the GLOBAL cell
+// index.  One slab = the handle's own grid.  With several, the other slabs' arrays are peer memory
+// (NVLink) or other handles on the same device.
+constexpr int MAX_SLABS = 8;
+template <typename T>
+struct SlabTab {
+    int n, rows;
+    const T *h[2][MAX_SLABS], *qx[2][MAX_SLABS], *qy[2][MAX_SLABS];   // [flood parity][slab]
+    uint8_t *occ[2][MAX_SLABS];                                          // [N_p buffer][slab]
+    __device__ __forceinline__ int of(int c, int nx) const { return n == 1 ? 0 : min((c / nx) / rows, n - 1); }
+};
+
 template <typename T>
 struct PedArgs {
     int n;                           // all agents, active or not
@@ -39,13 +52,12 @@ struct PedArgs {
     // N_p per cell is double-buffered by flood parity: the binning chain of step n+1 runs beside the
     // flood step n, which is still reading the N_p of step n (buffer ctl->parity)
     int32_t *cellprev;               // [2][n] per slot: cell whose occupancy this slot set the last time this buffer was filled, or -1
-    uint8_t *occ;                    // [2][ncell] N_p, saturated at 255
-    size_t cellprev_stride, occ_stride;
+    size_t cellprev_stride;
     int pdl_early;                   // 1: let the next kernel of the chain be scheduled at once (large crowds), see pdl_trigger()
     int pipelined;                   // 1: fill buffer ctl->occ_next (published by the pedestrian step of the step before); 0: ctl->parity
     const uint8_t *mask;             // [ncell] 1 = solid
     const uint8_t *nav;              // [n_targets][ncell]
-    const T *h[2], *qx[2], *qy[2];   // flood state (level n is [ctl->parity])
+    SlabTab<T> slab;                 // flood state (level n is [ctl->parity]) and N_p of every cell
     Ctl *ctl;
 };
 
@@ -89,7 +101,7 @@ __device__ __forceinline__ void bin_count_one(const PedArgs<T> &a, const int s, 
     a.A.cell[s] = cell;
     if (clear_occ) {
         const int c = a.cellprev[sel * a.cellprev_stride + s];
-        if (c >= 0) a.occ[sel * a.occ_stride + c] = 0;      // sparse clear: only cells that were set (no dense memset)
+        if (c >= 0) a.slab.occ[sel][a.slab.of(c, a.nx)][c] = 0;      // sparse clear: only cells that were set (no dense memset)
     }
 }
 
@@ -255,7 +267,7 @@ __global__ void __launch_bounds__(256) ped_occ_kernel(PedArgs<T> a)
     int same = 0, lower = 0;
     for (int j = a.start[b]; j < a.start[b + 1]; ++j)
         if (a.B.cell[j] == c) { same += 1; lower += (j < d); }
-    if (lower == 0) a.occ[sel * a.occ_stride + c] = (uint8_t)min(same, 255);
+    if (lower == 0) a.slab.occ[sel][a.slab.of(c, a.nx)][c] = (uint8_t)min(same, 255);
     cellprev[d] = c;
 }
 
@@ -365,9 +377,10 @@ __device__ __forceinline__ void ped_step_one(const PedArgs<T> &a, const int d)
     }
     // 1. sample U^n at the containing cell -> HR -> Table 1 (C17-C20)
     const int p = a.ctl->parity;
-    const T h = a.h[p][c];
+    const int sl = a.slab.of(c, a.nx);
+    const T h = a.slab.h[p][sl][c];
     T u = T(0), v = T(0);
-    if (h > a.h_dry) { u = div_rn(a.qx[p][c], h); v = div_rn(a.qy[p][c], h); }
+    if (h > a.h_dry) { u = div_rn(a.slab.qx[p][sl][c], h); v = div_rn(a.slab.qy[p][sl][c], h); }
     const T hr = mul_rn(add_rn(fmax(fabs(u), fabs(v)), T(0.5)), h);
     if (!(h > a.h_dry)) state = 0;
     else if (hr < a.hr_edge[0]) state = 1;
@@ -449,7 +462,8 @@ __global__ void __launch_bounds__(PED_THREADS) ped_step_kernel(PedArgs<T> a, int
 template <typename T>
 struct TailArgs {
     Ctl *ctl;
-    T *zs;
+    T *zs_tab[MAX_SLABS];            // bed of every row slab, pre-offset for the global cell index (8f-4)
+    int slab_rows, nx;
     const int32_t *line_cells;
     int n_line, bags_per_cell_layer, n_layers;
     T layer_thickness;
@@ -458,7 +472,7 @@ struct TailArgs {
     double inv_inflow_length;
     // entrance doors
     PedSoA<T> A;                     // level n+1 pedestrians (after the pedestrian step of this step)
-    int np, n_doors, nx;
+    int np, n_doors;
     int door_cells[16];
     double *door_credit;             // [16] newcomers owed by each door
     double spawn_rate, vpref_lo, vpref_hi, dx, dy;
@@ -583,7 +597,8 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
             for (int d = 0; d < D && !l.complete; ++d) {
                 l.bags += 1;
                 if (l.bags == a.bags_per_cell_layer) {
-                    a.zs[a.line_cells[l.cursor]] += a.layer_thickness;
+                    const int lc = a.line_cells[l.cursor];
+                    a.zs_tab[lc / a.nx / a.slab_rows][lc] += a.layer_thickness;
                     l.bags = 0; l.cursor += 1;
                     if (l.cursor == a.n_line) { l.layer += 1; l.cursor = 0; }
                     if (l.layer == a.n_layers) l.complete = 1;
@@ -612,6 +627,17 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
         c->halt = (l.t >= l.t_end) ? 1 : 0;
         c->q_in = q_in;
     }
+}
+
+// Row slabs: the global time step is the minimum over the slabs, i.e. the
+// maximum of their wave speeds: every slab's control block receives the maximum over all of them.
+struct SlabCtls { Ctl *c[MAX_SLABS]; int n; };
+__global__ void slab_lambda_kernel(SlabCtls t)
+{
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    unsigned long long m = 0ull;
+    for (int r = 0; r < t.n; ++r) { const unsigned long long v = t.c[r]->lam_bits; m = v > m ? v : m; }   // non-negative doubles order like integers
+    for (int r = 0; r < t.n; ++r) t.c[r]->lam_bits = m;
 }
 
 // ---------------------------------------------------------------------------------- read-back

@@ -157,3 +157,31 @@ def main(argv=None):
 
 if __name__ == "__main__":
     main()
+
+
+# ---------------------------------------------------------------------------- row slabs
+# Host logic of the row-slab decomposition (include/floodped.h sim_slab_link): which rows a slab
+# holds, which slab holds a row, and the one collective of the data path -- the global time step is
+# the minimum over the slabs, i.e. a MAX reduction of the slabs' wave speeds.
+
+def slab_cuts(ny: int, n_slabs: int) -> list[tuple[int, int]]:
+    """(first row, number of rows) per slab: equal slabs of ceil(ny / n) rows, the last one shorter;
+    fewer slabs than asked when ny is small.  This is the layout sim_slab_link checks."""
+    if ny <= 0 or n_slabs <= 0:
+        raise ValueError("ny and n_slabs must be positive")
+    rows = -(-ny // n_slabs)
+    return [(j0, min(rows, ny - j0)) for j0 in range(0, ny, rows)]
+
+
+def slab_of_row(row: int, ny: int, n_slabs: int) -> int:
+    """index of the slab that holds `row` (what the pedestrian kernels compute per agent)"""
+    cuts = slab_cuts(ny, n_slabs)
+    if not (0 <= row < ny):
+        raise ValueError("row outside the grid")
+    return min(row // cuts[0][1], len(cuts) - 1)
+
+
+def global_wave_speed(local_lambda: float, device=None) -> float:
+    """max over the slabs of max_cells (|u| + c) / dx: every rank then derives the same
+    dt = min(dt_max, CFL / lambda).  One 8-byte all-reduce per step."""
+    return max_over_ranks(local_lambda, device)

@@ -82,3 +82,46 @@ def test_shards_partition_any_size():
             parts = [replicas.shard(n, r, ws) for r in range(ws)]
             assert sorted(sum(parts, [])) == list(range(n))
             assert max(map(len, parts)) - min(map(len, parts)) <= 1
+
+
+# ---------------------------------------------------------------------------- row slabs
+
+def _slab_worker(rank, world_size, port, out_dir):
+    import json
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    from paper_1908_05232_b200 import replicas as R
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world_size)
+    try:
+        ny = 8191                                              # not divisible: the last slab is shorter
+        cut = R.slab_cuts(ny, world_size)[rank]
+        cuts = [None] * world_size
+        dist.all_gather_object(cuts, cut)
+        lam = R.global_wave_speed([3.25, 7.5][rank])           # rank 1 holds the fastest cell
+        dt = min(0.1, 0.5 / lam)
+        with open(os.path.join(out_dir, f"s{rank}.json"), "w") as f:
+            json.dump(dict(cut=cut, cuts=cuts, lam=lam, dt=dt), f)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_slab_partition_and_global_dt_world_size_2(tmp_path):
+    import json
+    import torch.multiprocessing as mp
+    port = _free_port()
+    mp.spawn(_slab_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    r0 = json.load(open(tmp_path / "s0.json")); r1 = json.load(open(tmp_path / "s1.json"))
+    assert r0["cuts"] == r1["cuts"] == [[0, 4096], [4096, 4095]]   # contiguous, in order, cover the grid
+    assert r0["lam"] == r1["lam"] == 7.5 and r0["dt"] == r1["dt"] == 0.5 / 7.5
+
+
+def test_slab_cuts_cover_any_grid_and_owner_lookup():
+    for ny in (1, 2, 7, 64, 8191, 8192):
+        for n in (1, 2, 3, 8):
+            cuts = replicas.slab_cuts(ny, n)
+            assert cuts[0][0] == 0 and sum(c[1] for c in cuts) == ny and len(cuts) <= n
+            assert all(cuts[k][0] + cuts[k][1] == cuts[k + 1][0] for k in range(len(cuts) - 1))
+            assert all(c[1] == cuts[0][1] for c in cuts[:-1]) and 0 < cuts[-1][1] <= cuts[0][1]
+            for row in {0, ny // 2, ny - 1}:
+                r = replicas.slab_of_row(row, ny, n)
+                assert cuts[r][0] <= row < cuts[r][0] + cuts[r][1]
