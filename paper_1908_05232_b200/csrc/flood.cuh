@@ -456,10 +456,10 @@ __global__ void flood_bed_kernel(const T *__restrict__ zs, const T *__restrict__
 // After a state re-injection (sim_write_flood): bed with the solid cells marked (z given: new bed;
 // else keep), and no water in solid cells (C16).
 template <typename T>
-__global__ void flood_inject_kernel(T *h, T *qx, T *qy, T *zs, const T *z_new, const uint8_t *mask, size_t n)
+__global__ void flood_inject_kernel(T *h, T *qx, T *qy, T *zs, const T *z_new, size_t n)
 {
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += (size_t)gridDim.x * blockDim.x) {
-        const bool solid = mask[c] != 0;
+        const bool solid = is_solid(zs[c]);            // solid cells are the cells with z = +inf, for good (R3)
         if (z_new) zs[c] = solid ? solid_z<T>() : z_new[c];
         if (solid) { h[c] = T(0); qx[c] = T(0); qy[c] = T(0); }
     }

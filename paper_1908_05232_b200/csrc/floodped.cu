@@ -1125,7 +1125,7 @@ template <typename T> int write_flood_t(sim *s, const void *h, const void *qx, c
     if (z) CU(cudaMemcpyAsync(s->scratch_real[0], z, bytes, cudaMemcpyHostToDevice, s->stream));
     // solid cells hold no water and keep z = +inf; then the CFL dt, q_in and halt of the injected state
     flood_inject_kernel<T><<<1184, 256, 0, s->stream>>>((T *)s->h[p], (T *)s->qx[p], (T *)s->qy[p], (T *)s->zs,
-                                                       z ? (const T *)s->scratch_real[0] : nullptr, s->mask, nc);
+                                                       z ? (const T *)s->scratch_real[0] : nullptr, nc);
     CU(cudaGetLastError());
     int rc = refresh_dt<T>(s);
     if (rc != SIM_OK) return rc;
