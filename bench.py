@@ -113,12 +113,13 @@ def scenario(cfg):
 ORACLE_STEPS = {1: 1000, 2: 2000, 3: 2000, 4: 20, 5: 5}
 
 
-def oracle_run(cfg, steps, warmup, sc=None):
+def oracle_run(cfg, steps, warmup, sc=None, flood_order=1):
     """The oracle as it stands, single thread, on the SAME workload (full size), over a bounded
     number of coupled steps; returns (cells/s, agents/s, s/step, desc)."""
     import oracle
     if sc is None:
         sc = scenario(cfg)
+        sc.flood_order = flood_order
     o = oracle.Oracle(sc)
     if warmup:
         o.step(warmup)
@@ -137,7 +138,7 @@ def run_reference(args):
         return
     steps = min(args.steps, ORACLE_STEPS[args.config])
     warm = min(args.warmup, 1)
-    cps, aps, sps, desc = oracle_run(args.config, steps, warm)
+    cps, aps, sps, desc = oracle_run(args.config, steps, warm, flood_order=args.flood_order)
     done_steps = steps
     line = {
         "impl": "reference", "metric": "flood cell-updates/s (coupled step)", "value": cps, "unit": "cell-updates/s",
@@ -175,6 +176,7 @@ def run_ours(args):
     build.build()
     K, W = args.steps, max(args.warmup, 3)
     sc = scenario(args.config)
+    sc.flood_order = args.flood_order
     real = np.float32 if sc.real_bits == 32 else np.float64
     ncell, npeds = sc.nx * sc.ny, sc.n_peds
     g = binding.Sim(sc, device=f"cuda:{local}")
@@ -297,7 +299,7 @@ def run_ours(args):
     else:
         cpu = None
 
-    kernel_name = ("flood_cell_kernel", "flood_tile_kernel", "flood_march_kernel", "flood_march2_kernel", "flood_tmarch_kernel")[variant]
+    kernel_name = ("flood_cell_kernel", "flood_tile_kernel", "flood_march_kernel", "flood_march2_kernel", "flood_tmarch_kernel", "flood_muscl_kernel")[variant]
     traffic, traffic_src = ncu_traffic(args.config, kernel_name) if args.march_rows == 0 and args.flood_variant < 0 else (None, None)
     agg = aggregate(ms_max, world, ncell, done, active)
     line = {
@@ -311,7 +313,7 @@ def run_ours(args):
         "config": {"workload": f"config{args.config}: {sc.name}", "nx": sc.nx, "ny": sc.ny, "dx": sc.dx,
                    "pedestrians": npeds, "active_pedestrians": active,
                    "l2_policy": "inputs larger than L2 (no flush)" if ncell * fb > 126e6 else "working set fits L2: latency-bound config, roofline not meaningful",
-                   "flood_variant": variant, "overlap_ped_flood": not args.no_overlap, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+                   "flood_variant": variant, "flood_order": args.flood_order, "overlap_ped_flood": not args.no_overlap, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": world * ncell * e2e_done / e2e_s, "unit": "cell-updates/s",
                 "h2d_bytes_per_step": h2d / e2e_done, "d2h_bytes_per_step": d2h / e2e_done,
@@ -349,6 +351,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--flood-variant", type=int, default=-1, choices=list(range(-1, 5)), help="-1: the library default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flood-order", type=int, default=1, choices=[1, 2], help="1: the paper's first-order flood step; 2: MUSCL-Hancock (SURVEY 8f-2)")
     ap.add_argument("--march-rows", type=int, default=0, help="rows per chunk of the row-marching flood kernel (0: library default)")
     ap.add_argument("--no-overlap", action="store_true", help="pedestrian step and flood step in one chain instead of parallel graph branches")
     args = ap.parse_args()

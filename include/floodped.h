@@ -175,11 +175,6 @@ int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const void *manni
 /* Enqueue n coupled steps on the stream; asynchronous; dt and t stay on the device. */
 int sim_step(sim_t *s, int64_t n);
 
-/* The same n steps launched kernel by kernel (no graph) with a CUDA event before each launch;
- * synchronises.  kernel_ms[8] receives the summed device time in ms of: 0 bin count, 1 bin scan,
- * 2 scatter, 3 pedestrian step, 4 flood step, 5 tail, 6 occupancy (N_p per cell); 7 unused.  For measurement. */
-int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms);
-
 /* Flood agents' recorded fields: depth, velocities (0 where h <= h_dry, C8), bed,
  * hazard rate.  Each [ny*nx] real; any pointer may be NULL. */
 int sim_read_flood(sim_t *s, void *h, void *u, void *v, void *z, void *hr);
@@ -193,7 +188,37 @@ int sim_read_peds(sim_t *s, void *x, void *y, void *vx, void *vy, uint8_t *state
                   uint8_t *active, int32_t *cell, void *timer);
 int sim_get_stats(sim_t *s, sim_stats_t *out);
 
-/* ---- test hooks ---- */
+/* ---- row slabs across GPUs (SURVEY 8f-4, S:8e) ----
+ * The flood grid is cut into n <= 8 slabs of whole rows, one handle per slab, in row order, each on
+ * its own device (or, for testing, several on one device); all slabs but the last have the same
+ * number of rows.  sim_slab_link makes the handles one simulation:
+ *   - the flood kernel of a slab reads the one halo row it needs from the neighbour slab IN PLACE
+ *     (peer memory: the handles must be in one process with peer access, which this call enables;
+ *     no halo buffers, no exchange kernel); P:L97 "immediate neighbours";
+ *   - the global time step is the minimum over the slabs: one 8-byte max-reduction of the wave
+ *     speed per step (P:L174);
+ *   - all pedestrians live on handles[0] (the other handles are created with n = 0): its
+ *     pedestrian kernels sample depth and velocity of whichever slab holds the cell, write N_p
+ *     there (P:L136-138) and raise the bed there (P:L146), again in place.
+ * Flood kernels: variant 4 (nx % 16 == 0) or 0.  Not combined with open edges or flood_order 2.
+ * sim_slab_step advances all slabs by n coupled steps (host-sequenced launches on the handles'
+ * streams, events between them; no kernel waits on another); sim_step on a linked handle fails.
+ * Results are bit-identical to the single-handle run of the whole grid. */
+int sim_slab_link(sim_t *const *handles, int32_t n);
+int sim_slab_step(sim_t *const *handles, int32_t n, int64_t steps);
+
+/* ============================================================================================
+ * Everything above is the product ABI of SURVEY 8(b).  Below: TEST AND TUNING HOOKS -- state
+ * re-injection for the parity tests, kernel selection and per-kernel timing for measurement.
+ * A user of the simulator needs none of them.  (SURVEY 8(b) deviations, recorded in DESIGN.md 1:
+ * sim_read_peds / sim_write_peds take separate arrays incl. `active` and `timer`.)
+ * ============================================================================================ */
+/* The same n steps launched kernel by kernel (no graph) with a CUDA event before each launch;
+ * synchronises.  kernel_ms[8] receives the summed device time in ms of: 0 bin count, 1 bin scan,
+ * 2 scatter, 3 pedestrian step, 4 flood step, 5 tail, 6 occupancy (N_p per cell); 7 unused.  For measurement. */
+int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms);
+
+
 /* Bin the pedestrians of the current level without stepping: key[n] in original order (bin
  * index, n_bins for inactive), order[n] = original index held by each sorted slot,
  * start[n_bins+2] exclusive scan (start[n_bins+1] = n).  Bins are k x k cells,
@@ -225,25 +250,6 @@ int sim_set_march_rows(sim_t *s, int32_t rows);
 int sim_set_overlap(sim_t *s, int32_t on);
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
-
-/* ---- row slabs across GPUs (SURVEY 8f-4, S:8e) ----
- * The flood grid is cut into n <= 8 slabs of whole rows, one handle per slab, in row order, each on
- * its own device (or, for testing, several on one device); all slabs but the last have the same
- * number of rows.  sim_slab_link makes the handles one simulation:
- *   - the flood kernel of a slab reads the one halo row it needs from the neighbour slab IN PLACE
- *     (peer memory: the handles must be in one process with peer access, which this call enables;
- *     no halo buffers, no exchange kernel); P:L97 "immediate neighbours";
- *   - the global time step is the minimum over the slabs: one 8-byte max-reduction of the wave
- *     speed per step (P:L174);
- *   - all pedestrians live on handles[0] (the other handles are created with n = 0): its
- *     pedestrian kernels sample depth and velocity of whichever slab holds the cell, write N_p
- *     there (P:L136-138) and raise the bed there (P:L146), again in place.
- * Flood kernels: variant 4 (nx % 16 == 0) or 0.  Not combined with open edges or flood_order 2.
- * sim_slab_step advances all slabs by n coupled steps (host-sequenced launches on the handles'
- * streams, events between them; no kernel waits on another); sim_step on a linked handle fails.
- * Results are bit-identical to the single-handle run of the whole grid. */
-int sim_slab_link(sim_t *const *handles, int32_t n);
-int sim_slab_step(sim_t *const *handles, int32_t n, int64_t steps);
 
 const char *sim_last_error(const sim_t *s);     /* s may be NULL: error of the last failed create */
 void sim_destroy(sim_t *s);
