@@ -494,6 +494,8 @@ template <typename T> int build_graph(sim *s, int level)
     e = cudaGraphInstantiate(&ex, g, 0);
     cudaGraphDestroy(g);
     if (e != cudaSuccess) return fail(s, SIM_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
+    e = cudaGraphUpload(ex, s->stream);              // so that the first replay of a ladder level costs what every replay costs
+    if (e != cudaSuccess) { cudaGraphExecDestroy(ex); return fail(s, SIM_ECUDA, std::string("graph upload: ") + cudaGetErrorString(e)); }
     s->graph[level] = ex;
     return SIM_OK;
 }
