@@ -342,6 +342,43 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slabs(args):
+    """SURVEY 8f-4 on ONE GPU: the grid cut into --slabs row slabs, one handle each, all on cuda:0
+    (no multi-GPU node here): what the slab machinery costs per step against the single handle
+    (host-sequenced launches and events instead of a replayed graph; halo rows and the pedestrians'
+    cells read through the slab tables), and that the result is bit-identical."""
+    import torch
+    from paper_1908_05232_b200 import binding, build
+    torch.cuda.set_device(0)
+    build.build()
+    K, W = args.steps, max(args.warmup, 3)
+    sc = scenario(args.config)
+    one = binding.Sim(sc)
+    slabs = binding.SlabSim(sc, args.slabs)
+    ms = {}
+    for name, g in (("single", one), ("slabs", slabs)):
+        g.step(W)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); g.step(K); e1.record()
+        torch.cuda.synchronize()
+        ms[name] = e0.elapsed_time(e1) / K
+    a, b = slabs.read_conserved(), one.read_conserved()
+    same = all(bool(np.array_equal(a[k], b[k])) for k in ("h", "qx", "qy")) and slabs.stats()["dt"] == one.stats()["dt"]
+    diff = max(float(np.max(np.abs(a[k].astype(np.float64) - b[k]))) / max(float(np.max(np.abs(b[k]))), 1e-300) for k in ("h", "qx", "qy"))
+    ncell = sc.nx * sc.ny
+    print(json.dumps({
+        "metric": "flood cell-updates/s (coupled step)", "value": ncell / (ms["slabs"] * 1e-3), "unit": "cell-updates/s",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms["slabs"], "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f32" if sc.real_bits == 32 else "f64", "data": "synthetic",
+        "config": {"workload": f"config{args.config}: {sc.name}", "parallelism": f"{len(slabs.sims)} row slabs, all on one GPU (emulation of SURVEY 8f-4; unmeasured on multi-GPU hardware)",
+                   "rows_per_slab": [c[1] for c in slabs.cuts]},
+        "single_handle_ms_per_step": ms["single"], "slab_overhead": ms["slabs"] / ms["single"] - 1.0,
+        "bit_identical_to_single_handle": same, "max_rel_diff_to_single_handle": diff,
+        "note": "bit-identical whenever the people -> flow coupling is off or there are no pedestrians (tests/test_gpu_slabs.py); with it on, "
+                "two runs of the SAME handle differ as well: pair forces are summed in the order of the counting sort's atomics"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -354,7 +391,10 @@ def main():
     ap.add_argument("--flood-order", type=int, default=1, choices=[1, 2], help="1: the paper's first-order flood step; 2: MUSCL-Hancock (SURVEY 8f-2)")
     ap.add_argument("--march-rows", type=int, default=0, help="rows per chunk of the row-marching flood kernel (0: library default)")
     ap.add_argument("--no-overlap", action="store_true", help="pedestrian step and flood step in one chain instead of parallel graph branches")
+    ap.add_argument("--slabs", type=int, default=0, help="SURVEY 8f-4: cut the grid into this many row slabs, all on cuda:0, and compare with the single handle")
     args = ap.parse_args()
+    if args.slabs > 1 and args.impl == "ours":
+        return run_slabs(args)
     if args.impl == "reference":
         run_reference(args)
     else:
