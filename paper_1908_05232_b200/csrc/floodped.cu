@@ -334,7 +334,8 @@ template <typename T> PedArgs<T> ped_args_full(const sim *s, int pipelined)
         pa.door_target[d] = s->door_target[d];
     }
     pa.pipelined = pipelined;
-    pa.pdl_early = s->np >= 65536;   // measured: pre-scheduling the chain pays on Config 5 (-1.5 %), costs on Configs 1-3 (+8 %)
+    pa.pdl_early = s->np >= 65536;
+    pa.occ_in_scatter = s->np < 65536;   // small crowds are launch-bound: four dependent launches per step instead of five   // measured: pre-scheduling the chain pays on Config 5 (-1.5 %), costs on Configs 1-3 (+8 %)
     return pa;
 }
 
@@ -359,7 +360,7 @@ template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelin
     mark();
     CU(launch_pdl(ped_scatter_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
     mark();
-    CU(launch_pdl(ped_occ_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
+    if (!pa.occ_in_scatter) CU(launch_pdl(ped_occ_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
     CU(cudaGetLastError());
     return SIM_OK;
 }
@@ -812,7 +813,7 @@ extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
     return DISPATCH(s, step_profiled, s, n, kernel_ms);
 }
 
-extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? (s->overlap ? 6 : 7) : 2) : 0; }
+extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? (s->overlap ? 6 : 7) - (s->np < 65536 ? 1 : 0) : 2) : 0; }
 
 extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
 {

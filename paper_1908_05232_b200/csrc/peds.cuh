@@ -53,6 +53,7 @@ struct PedArgs {
     // flood step n, which is still reading the N_p of step n (buffer ctl->parity)
     int32_t *cellprev;               // [2][n] per slot: cell whose occupancy this slot set the last time this buffer was filled, or -1
     size_t cellprev_stride;
+    int occ_in_scatter;              // 1 (small crowds): the scatter kernel counts N_p itself, no ped_occ_kernel launch
     int pdl_early;                   // 1: let the next kernel of the chain be scheduled at once (large crowds), see pdl_trigger()
     int pipelined;                   // 1: fill buffer ctl->occ_next (published by the pedestrian step of the step before); 0: ctl->parity
     const uint8_t *mask;             // [ncell] 1 = solid
@@ -244,6 +245,25 @@ __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
     a.B.vpref[d] = a.A.vpref[s]; a.B.timer[d] = a.A.timer[s];
     a.B.role[d] = a.A.role[s]; a.B.fsm[d] = a.A.fsm[s]; a.B.state[d] = a.A.state[s];
     a.B.active[d] = a.A.active[s]; a.B.id[d] = a.A.id[s]; a.B.cell[d] = a.A.cell[s];
+    // small crowds: N_p per cell here, one launch fewer on the critical path of the step.
+    // Saturating add of 1 to the cell's byte by compare-and-swap on its word (the cells that were set
+    // the last time this buffer was filled have been cleared by the count kernel before).
+    if (a.occ_in_scatter) {
+        const int sel = chain_sel(a);
+        int32_t *cellprev = a.cellprev + sel * a.cellprev_stride;
+        if (!a.A.active[s]) { cellprev[d] = -1; return; }
+        const int c = a.A.cell[s];
+        uint8_t *p = a.slab.occ[sel][a.slab.of(c, a.nx)] + c;
+        unsigned int *w = reinterpret_cast<unsigned int *>(reinterpret_cast<uintptr_t>(p) & ~uintptr_t(3));
+        const int sh = 8 * (int)(reinterpret_cast<uintptr_t>(p) & 3);
+        unsigned int old = *w;
+        while (((old >> sh) & 255u) != 255u) {
+            const unsigned int seen = atomicCAS(w, old, old + (1u << sh));
+            if (seen == old) break;
+            old = seen;
+        }
+        cellprev[d] = c;
+    }
 }
 
 // ---------------------------------------------------------------------------------- (O)
