@@ -248,6 +248,10 @@ int sim_set_march_rows(sim_t *s, int32_t rows);
 /* 1 (default): the pedestrian step runs as a parallel branch of the step graph beside the flood
  * step (both read level n only); 0: every kernel of the step in one chain.  Same results. */
 int sim_set_overlap(sim_t *s, int32_t on);
+/* 1 (default): the TMA march kernel skips chunks whose cells, and whose neighbour segments, hold exact
+ * zeros (dry ground: every flux is zero, the result is zeros), reading and writing nothing for them;
+ * 0: every chunk is computed.  Same results bit for bit. */
+int sim_set_dry_skip(sim_t *s, int32_t on);
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
 

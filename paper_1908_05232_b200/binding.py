@@ -19,7 +19,7 @@ SIM_OK, SIM_EINVAL, SIM_ENOMEM, SIM_ECUDA, SIM_ENOTFINITE = 0, -1, -2, -3, -4
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
-    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap",
+    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap", "sim_set_dry_skip",
     "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_last_error", "sim_destroy",
 ]
 
@@ -118,6 +118,7 @@ def load_library(path: str = LIB_PATH):
     L.sim_get_flood_variant.argtypes = [_vp]
     L.sim_set_march_rows.argtypes = [_vp, C.c_int32]
     L.sim_set_overlap.argtypes = [_vp, C.c_int32]
+    L.sim_set_dry_skip.argtypes = [_vp, C.c_int32]
     L.sim_kernels_per_step.argtypes = [_vp]
     L.sim_slab_link.argtypes = [C.POINTER(_vp), C.c_int32]
     L.sim_slab_step.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int64]
@@ -283,6 +284,9 @@ class Sim:
 
     def set_overlap(self, on):
         self._chk(self._L.sim_set_overlap(self._h, int(bool(on))))
+
+    def set_dry_skip(self, on):
+        self._chk(self._L.sim_set_dry_skip(self._h, int(bool(on))))
 
     def flood_variant(self) -> int:
         return self._L.sim_get_flood_variant(self._h)

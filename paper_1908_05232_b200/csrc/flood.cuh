@@ -40,6 +40,8 @@ struct FloodArgs {
     // [0 south | 1 north][flood parity]; null = the domain edge (wall ghost).  Kernels 0 and 4.
     const T *halo_h[2][2], *halo_qx[2][2], *halo_qy[2][2];
     const T *halo_z[2];
+    uint8_t *dryseg;                  // TMA march kernel: [2][chunk rows][nsegx] dry-segment flags (see flood_tmarch_kernel); null = off
+    size_t dry_stride; int nsegx;
     int open_sides;                   // bit per domain edge (W, E, S, N): open, transmissive ghost; kernels 0 and 5 only
     Ctl *ctl;
 };

@@ -70,6 +70,7 @@ struct sim {
     int flood_variant = 1;
     int march_R = 64, march_gx = 1, march_gy = 1;
     uint8_t *chunk_flag = nullptr;
+    uint8_t *dryseg = nullptr; size_t dry_stride = 0; int nsegx = 0; int dry_skip = 1;   // dry-segment flags of the TMA march kernel
     void *ghost_zero = nullptr, *ghost_inf = nullptr;   // one strip-wide row each (TMA kernel, rows beyond the domain)
     int exit_i[16]{}, exit_j[16]{};
     int door_cells[16]{}, door_target[16]{};
@@ -146,6 +147,8 @@ size_t layout(sim *s, Bump &b)
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
     s->ghost_zero = b.take<double>(MW); s->ghost_inf = b.take<double>(MW);
     s->chunk_flag = b.take<uint8_t>((size_t)s->march_gx * ((s->grid.ny + 7) / 8));    // room for any R >= 8
+    s->nsegx = (s->grid.nx + 63) / 64; s->dry_stride = (size_t)s->nsegx * ((s->grid.ny + 7) / 8 + 2);
+    s->dryseg = b.take<uint8_t>(2 * s->dry_stride);
     s->scan_status = b.take<unsigned long long>((size_t)(s->nbins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1);
     return (b.off + 255) & ~size_t(255);
 }
@@ -233,6 +236,7 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     a.chunk_flag = s->chunk_flag; a.R = s->march_R;
     a.ghost_zero = (const T *)s->ghost_zero; a.ghost_inf = (const T *)s->ghost_inf; a.ghost_occ = (const uint8_t *)s->ghost_zero;
     a.open_sides = s->prm.open_sides;
+    a.dryseg = s->dry_skip ? s->dryseg : nullptr; a.dry_stride = s->dry_stride; a.nsegx = s->nsegx;
     if (s->ngroup > 1) {
         const size_t nx = (size_t)s->grid.nx;
         const sim *lo = s->grank > 0 ? s->group[s->grank - 1] : nullptr, *hi = s->grank + 1 < s->ngroup ? s->group[s->grank + 1] : nullptr;
@@ -824,6 +828,7 @@ extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
     s->march_R = rows;
     s->march_gy = (s->grid.ny + rows - 1) / rows;
     drop_graphs(s);
+    CU(cudaMemsetAsync(s->dryseg, 0, 2 * s->dry_stride, s->stream));       // the flags are per chunk row of R rows
     if (s->grid.real_bits == 32)
         flood_chunk_flags_kernel<float><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const float *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
     else
@@ -961,6 +966,7 @@ extern "C" int sim_slab_link(sim_t *const *h, int32_t n)
         q->ngroup = n; q->grank = r;
         for (int k = 0; k < n; ++k) q->group[k] = h[k];
         if (q->flood_variant != 0 && q->flood_variant != 4) q->flood_variant = q->grid.nx % 16 == 0 ? 4 : 0;
+        CU(cudaMemsetAsync(q->dryseg, 0, 2 * q->dry_stride, q->stream));
         if (!q->ev_slab) CU(cudaEventCreateWithFlags(&q->ev_slab, cudaEventDisableTiming));
         q->binned = false;
     }
@@ -1008,6 +1014,18 @@ extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
     CU(cudaStreamSynchronize(s->stream));
     s->flood_variant = variant;
     drop_graphs(s);
+    CU(cudaMemsetAsync(s->dryseg, 0, 2 * s->dry_stride, s->stream));       // only the TMA march kernel keeps the dry flags up to date
+    return SIM_OK;
+}
+
+extern "C" int sim_set_dry_skip(sim_t *s, int32_t on)
+{
+    if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
+    CU(cudaStreamSynchronize(s->stream));
+    s->dry_skip = on ? 1 : 0;
+    drop_graphs(s);
+    CU(cudaMemsetAsync(s->dryseg, 0, 2 * s->dry_stride, s->stream));
     return SIM_OK;
 }
 
@@ -1127,6 +1145,7 @@ template <typename T> int write_flood_t(sim *s, const void *h, const void *qx, c
     if (qy) CU(cudaMemcpyAsync(s->qy[p], qy, bytes, cudaMemcpyHostToDevice, s->stream));
     if (z) CU(cudaMemcpyAsync(s->scratch_real[0], z, bytes, cudaMemcpyHostToDevice, s->stream));
     // solid cells hold no water and keep z = +inf; then the CFL dt, q_in and halt of the injected state
+    CU(cudaMemsetAsync(s->dryseg, 0, 2 * s->dry_stride, s->stream));       // state written from outside: nothing is known to be dry
     flood_inject_kernel<T><<<1184, 256, 0, s->stream>>>((T *)s->h[p], (T *)s->qx[p], (T *)s->qy[p], (T *)s->zs,
                                                        z ? (const T *)s->scratch_real[0] : nullptr, nc);
     CU(cudaGetLastError());
