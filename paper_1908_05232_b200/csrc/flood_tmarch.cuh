@@ -502,11 +502,9 @@ __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tma
     constexpr int NT = MW / CPT;
     __shared__ March2Smem<T, CPT> s;
     extern __shared__ __align__(16) unsigned char tm_dyn[];
-    if (a.ctl->halt) return;
     RowStage<T> *ring = reinterpret_cast<RowStage<T> *>(tm_dyn);
     uint64_t *bars = reinterpret_cast<uint64_t *>(tm_dyn + sizeof(RowStage<T>) * STAGES);
     const int x0 = blockIdx.x * MW, y0 = blockIdx.y * a.R;
-    const int path = a.chunk_flag[blockIdx.y * gridDim.x + blockIdx.x];
     const int tid = threadIdx.x;
     // ---- dry chunks.  dryseg[buffer][chunk row][64-column segment] = 1: every h, qx, qy of those R x 64 cells of
     // that ping-pong buffer is an exact zero (written by this kernel only; everything else that writes flood
@@ -515,25 +513,33 @@ __global__ void __launch_bounds__(MW / CPT, sizeof(T) == 4 ? MINB : 2) flood_tma
     // every flux is zero and level n+1 is zeros too (no inflow away from the domain edge): nothing to read.
     // If its segments of the OTHER buffer (level n-1) are flagged as well, there is nothing to write either
     // and the CTA ends here.  40 % of Config 5's cells are dry; 21 % of its chunks end this way.
+    // All loads of this prologue are independent (the flags of BOTH buffers are fetched, the parity picks),
+    // and every warp takes the decision for itself: one memory latency, no barrier.
+    const int lane = tid & 31, cy = blockIdx.y, sx0 = blockIdx.x * (MW / 64);
+    int f_a = 1, f_b = 1;                              // my flag of buffer 0 / buffer 1: lanes 0..13 inputs, lanes 16..19 own segments
+    if (a.dryseg) {
+        size_t idx = 0; bool have = false;
+        if (lane < 12) { idx = (size_t)(cy + lane / 4 - 1) * a.nsegx + sx0 + (lane & 3); have = cy > 0 && cy + 1 < (int)gridDim.y; }
+        else if (lane == 12) { idx = (size_t)cy * a.nsegx + sx0 - 1; have = sx0 > 0; }
+        else if (lane == 13) { idx = (size_t)cy * a.nsegx + sx0 + MW / 64; have = sx0 + MW / 64 < a.nsegx; }
+        else if (lane >= 16 && lane < 16 + MW / 64) { idx = (size_t)cy * a.nsegx + sx0 + (lane - 16); have = true; }
+        if (lane < 14 || (lane >= 16 && lane < 16 + MW / 64)) {
+            f_a = have ? a.dryseg[idx] : 0;
+            f_b = have ? a.dryseg[a.dry_stride + idx] : 0;
+        }
+    }
+    const int path = a.chunk_flag[blockIdx.y * gridDim.x + blockIdx.x];
+    const int2 hp = *reinterpret_cast<const int2 *>(&a.ctl->parity);     // parity, halt: adjacent in Ctl
+    if (hp.y) return;
     uint8_t *dry_out = nullptr;
     if (a.dryseg && (path == 0 || path == 2)) {
-        __shared__ int skip_s;
-        const int p = a.ctl->parity, cy = blockIdx.y, sx0 = blockIdx.x * (MW / 64);
-        const uint8_t *fin = a.dryseg + (size_t)p * a.dry_stride;
+        const int p = hp.x;
         dry_out = a.dryseg + (size_t)(p ^ 1) * a.dry_stride + (size_t)cy * a.nsegx + sx0;
-        if (tid < 32) {
-            int ok = 1, outok = 1;
-            if (tid < 12) ok = fin[(size_t)(cy + tid / 4 - 1) * a.nsegx + sx0 + (tid & 3)];
-            else if (tid == 12) ok = sx0 > 0 ? fin[(size_t)cy * a.nsegx + sx0 - 1] : 0;
-            else if (tid == 13) ok = sx0 + MW / 64 < a.nsegx ? fin[(size_t)cy * a.nsegx + sx0 + MW / 64] : 0;
-            if (tid < MW / 64) outok = dry_out[tid];
-            const bool in_dry = __all_sync(0xffffffffu, ok != 0), out_dry = __all_sync(0xffffffffu, outok != 0);
-            if (tid == 0) skip_s = in_dry ? (out_dry ? 2 : 1) : 0;
-        }
-        __syncthreads();
-        const int skip = skip_s;
-        if (skip == 2) return;
-        if (skip == 1) {                               // dried up since level n-1: write the zeros once
+        const int fin = p ? f_b : f_a, fout = p ? f_a : f_b;
+        const bool in_dry = __all_sync(0xffffffffu, lane >= 14 || fin != 0);
+        const bool out_dry = __all_sync(0xffffffffu, lane < 16 || lane >= 16 + MW / 64 || fout != 0);
+        if (in_dry && out_dry) return;
+        if (in_dry) {                                  // dried up since level n-1: write the zeros once
             const int p1 = p ^ 1;
             VecN<T, CPT> zero;
 #pragma unroll
