@@ -95,3 +95,18 @@ def test_row_slabs_with_the_skip_against_a_single_handle_without():
         for k in ("h", "qx", "qy"):
             assert np.array_equal(a[k], b[k]), k
         assert slabs.stats()["dt"] == off.stats()["dt"]
+
+
+def test_ragged_width_and_height_partial_strip_and_short_last_chunk():
+    """nx = 1072 = 4 full strips of 256 + a strip that sticks out of the domain (general path, never
+    flagged), ny = 301: a short last chunk; dry land on the right, a lake with a bump on the left"""
+    nx, ny = 1072, 301
+    j, i = np.mgrid[0:ny, 0:nx]
+    z = 0.4 * (i / nx)
+    h0 = np.maximum(0.0, 0.1 - z) + 0.05 * np.exp(-((i - 90) ** 2 + (j - 150) ** 2) / 300.0) * (z < 0.1)
+    for bits in (32, 64):
+        sc = box(nx, ny, dx=0.5, real_bits=bits, z=z, h0=h0, manning=0.02)
+        on, off = _pair(sc, rows=16)
+        for _ in range(5):
+            on.step(21); off.step(21)
+            _same(on, off)

@@ -117,3 +117,24 @@ def test_link_validation():
     g = binding.SlabSim(sc, 2)
     with pytest.raises(binding.FloodpedError):
         g.sims[0].step(1)
+
+
+def test_doors_and_trigger_on_slabs_match_the_oracle_step_by_step():
+    """the doors of SURVEY 8f-3 on a grid cut into two slabs: newcomers are placed by the first slab's
+    tail kernel, walk across the cut, the trigger comes from the maximum of BOTH slabs' wave speeds"""
+    from gpu_common import sync
+    sc = S.door_hall(n=64, slots=200, t_pre=20.0, spawn_rate=0.5, t_end=200.0)
+    o = oracle.Oracle(sc)
+    slabs = binding.SlabSim(sc, 2)
+    seen = False
+    for k in range(60):
+        o.step(1); slabs.step(1)
+        sa, sb = slabs.stats(), o.stats()
+        assert sa["spawned"] == sb["spawned"] and sa["triggered"] == sb["triggered"], k
+        pa, pb = slabs.read_peds(), o.read_peds()
+        if not seen:                       # dry phase: dt = dt_max on both sides, everything discrete is exact
+            assert np.array_equal(pa["active"], pb["active"]) and np.array_equal(pa["fsm"], pb["fsm"]), k
+        seen = seen or bool(sb["triggered"])
+    assert seen and sb["spawned"] > 20
+    rows = pb["cell"][pb["active"] == 1] // sc.nx
+    assert (rows < 32).any() and (rows >= 32).any()
