@@ -200,12 +200,35 @@ int sim_get_stats(sim_t *s, sim_stats_t *out);
  *   - all pedestrians live on handles[0] (the other handles are created with n = 0): its
  *     pedestrian kernels sample depth and velocity of whichever slab holds the cell, write N_p
  *     there and raise the bed there, again in place.
- * Flood kernels: variant 4 (nx % 16 == 0) or 0.  Not combined with open edges or flood_order 2.
+ * Flood kernels: variant 4 (nx a multiple of 256) or 0.  Not combined with open edges or flood_order 2.
  * sim_slab_step advances all slabs by n coupled steps (host-sequenced launches on the handles'
  * streams, events between them; no kernel waits on another); sim_step on a linked handle fails.
  * Results are bit-identical to the single-handle run of the whole grid. */
 int sim_slab_link(sim_t *const *handles, int32_t n);
 int sim_slab_step(sim_t *const *handles, int32_t n, int64_t steps);
+
+/* The same slabs with ONE PROCESS PER GPU (torch.distributed; binding.SlabRank).  A slab describes
+ * what it lends to the others -- device addresses in ITS address space and the base of its
+ * workspace; the other processes map that workspace (CUDA IPC: torch's shared CUDA tensors), rebase
+ * the addresses into their own address space and attach all n descriptions, their own included, in
+ * row order.  One step of a rank is then
+ *     sim_slab_enqueue(s, 0)   pedestrian step and binning chain of the next step (the rank that holds
+ *                              the pedestrians), then the flood kernel of this slab
+ *     all-reduce MAX over the ranks of the 8 bytes at `lam_bits` (NCCL; it is also the only barrier
+ *                              the step needs: every peer access of step n is ordered before it)
+ *     sim_slab_enqueue(s, 1)   tail: t += dt, next dt from the global wave speed
+ * and after attaching, once: sim_slab_enqueue(s, 2) (wave speed of the initial state), the same
+ * all-reduce, sim_slab_enqueue(s, 3).  No doors in this mode (newcomers are placed by the tail, after
+ * the binning chain has run). */
+typedef struct {
+    int32_t  j0, ny;                            /* rows [j0, j0 + ny) of the grid                     */
+    uint64_t h[2], qx[2], qy[2], zs, occ, ctl;  /* device addresses of the slab's arrays              */
+    uint64_t lam_bits;                          /* device address of the 8-byte wave-speed word       */
+    uint64_t workspace, workspace_bytes;        /* the allocation all of them live in                 */
+} sim_slab_desc_t;
+int sim_slab_describe(sim_t *s, sim_slab_desc_t *out);
+int sim_slab_attach(sim_t *s, int32_t rank, int32_t n, const sim_slab_desc_t *descs);
+int sim_slab_enqueue(sim_t *s, int32_t phase);
 
 /* ============================================================================================
  * Everything above is the product ABI of SURVEY 8(b).  Below: TEST AND TUNING HOOKS -- state

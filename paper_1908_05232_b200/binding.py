@@ -20,7 +20,7 @@ EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
     "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap", "sim_set_dry_skip",
-    "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_last_error", "sim_destroy",
+    "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_slab_describe", "sim_slab_attach", "sim_slab_enqueue", "sim_last_error", "sim_destroy",
 ]
 
 _vp = C.c_void_p
@@ -65,6 +65,32 @@ class SimParams(C.Structure):
         ("spawn_rate", C.c_double), ("target_population", C.c_int32), ("spawn_seed", C.c_uint64),
         ("spawn_vpref_lo", C.c_double), ("spawn_vpref_hi", C.c_double),
     ]
+
+
+class SlabDesc(C.Structure):
+    _fields_ = [("j0", C.c_int32), ("ny", C.c_int32),
+                ("h", C.c_uint64 * 2), ("qx", C.c_uint64 * 2), ("qy", C.c_uint64 * 2),
+                ("zs", C.c_uint64), ("occ", C.c_uint64), ("ctl", C.c_uint64), ("lam_bits", C.c_uint64),
+                ("workspace", C.c_uint64), ("workspace_bytes", C.c_uint64)]
+
+    ADDRS = ("zs", "occ", "ctl", "lam_bits")
+
+    def to_dict(self):
+        d = {k: int(getattr(self, k)) for k in ("j0", "ny", "workspace", "workspace_bytes") + self.ADDRS}
+        d.update({k: [int(v) for v in getattr(self, k)] for k in ("h", "qx", "qy")})
+        return d
+
+    @classmethod
+    def rebased(cls, d, new_base):
+        """the description `d` (a dict made by to_dict in the owner's process) with every address moved
+        from the owner's workspace base to `new_base`, where this process has that workspace mapped"""
+        o, delta = cls(), int(new_base) - int(d["workspace"])
+        o.j0, o.ny, o.workspace, o.workspace_bytes = d["j0"], d["ny"], int(new_base), d["workspace_bytes"]
+        for k in cls.ADDRS:
+            setattr(o, k, d[k] + delta)
+        for k in ("h", "qx", "qy"):
+            setattr(o, k, (C.c_uint64 * 2)(*[v + delta for v in d[k]]))
+        return o
 
 
 class SimStats(C.Structure):
@@ -122,6 +148,9 @@ def load_library(path: str = LIB_PATH):
     L.sim_kernels_per_step.argtypes = [_vp]
     L.sim_slab_link.argtypes = [C.POINTER(_vp), C.c_int32]
     L.sim_slab_step.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int64]
+    L.sim_slab_describe.argtypes = [_vp, C.POINTER(SlabDesc)]
+    L.sim_slab_attach.argtypes = [_vp, C.c_int32, C.c_int32, C.POINTER(SlabDesc)]
+    L.sim_slab_enqueue.argtypes = [_vp, C.c_int32]
     L.sim_last_error.argtypes = [_vp]
     L.sim_last_error.restype = C.c_char_p
     L.sim_destroy.argtypes = [_vp]
@@ -411,3 +440,76 @@ class SlabSim:
     def close(self):
         for g in self.sims:
             g.close()
+
+
+class SlabRank:
+    """One row slab per PROCESS and GPU (include/floodped.h sim_slab_attach), under an
+    initialised torch.distributed group: rank r holds slab r (rank 0 also all pedestrians).  The
+    workspaces are shared between the processes as CUDA-IPC tensors (torch.multiprocessing's
+    reductions), so that a slab's flood kernel reads its halo rows, and the pedestrian kernels read
+    and write the cells of other slabs, in place; the one collective per step is the MAX all-reduce of
+    the 8-byte wave speed (NCCL on the device; any other backend through a host copy, for tests).
+    Marshalling and sequencing only."""
+
+    def __init__(self, sc, device=None):
+        import torch
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        from .replicas import slab_cuts
+        self.rank, self.world = dist.get_rank(), dist.get_world_size()
+        cuts = slab_cuts(sc.ny, self.world)
+        if len(cuts) != self.world:
+            raise ValueError("fewer rows than ranks")
+        self.cut = cuts[self.rank]
+        self.sim = Sim(sc, device=device or f"cuda:{torch.cuda.current_device()}", slab=self.cut, with_peds=(self.rank == 0))
+        self._L = self.sim._L
+        mine = SlabDesc()
+        self.sim._chk(self._L.sim_slab_describe(self.sim._h, C.byref(mine)))
+        ws = self.sim._ws
+        assert ws.data_ptr() == mine.workspace
+        torch.cuda.synchronize()
+        offer = (mine.to_dict(), reduce_tensor(ws))
+        offers = [None] * self.world
+        dist.all_gather_object(offers, offer)
+        self._peers = []                                   # mapped workspaces of the other ranks: keep them alive
+        descs = (SlabDesc * self.world)()
+        for r, (d, (rebuild, args)) in enumerate(offers):
+            if r == self.rank:
+                descs[r] = mine
+            else:
+                t = rebuild(*args)                         # the peer's workspace, mapped into this process
+                self._peers.append(t)
+                descs[r] = SlabDesc.rebased(d, t.data_ptr())
+        self.sim._chk(self._L.sim_slab_attach(self.sim._h, self.rank, self.world, descs))
+        off = mine.lam_bits - mine.workspace
+        self._lam = ws[off:off + 8].view(torch.int64)      # bit pattern of a non-negative double: ordered like an integer
+        self._nccl = dist.get_backend() == "nccl"
+        dist.barrier()
+        self._phase(2); self._reduce(); self._phase(3)
+
+    def _phase(self, k):
+        self.sim._chk(self._L.sim_slab_enqueue(self.sim._h, int(k)))
+
+    def _reduce(self):
+        import torch
+        import torch.distributed as dist
+        if self._nccl:
+            dist.all_reduce(self._lam, op=dist.ReduceOp.MAX)
+        else:                                              # CPU backends (tests): through the host
+            torch.cuda.synchronize()
+            v = self._lam.cpu()
+            dist.all_reduce(v, op=dist.ReduceOp.MAX)
+            self._lam.copy_(v)
+            torch.cuda.synchronize()
+
+    def step(self, n=1):
+        for _ in range(int(n)):
+            self._phase(0); self._reduce(); self._phase(1)
+
+    def close(self):
+        import torch
+        import torch.distributed as dist
+        torch.cuda.synchronize()
+        dist.barrier()                                     # nobody unmaps a workspace another rank may still read
+        self.sim.close()
+        self._peers = []

@@ -46,7 +46,10 @@ struct sim {
     // row slab: the flood arrays hold rows [j0, j0 + grid.ny) of a grid of gny rows; the
     // pedestrians (all of them live on the first slab's handle) walk on the whole grid of pcell cells
     int gny = 0, j0 = 0, pcell = 0;
-    sim *group[8]{}; int ngroup = 0, grank = 0;   // linked slabs in row order (sim_slab_link)
+    // linked slabs in row order (sim_slab_link: handles of this process; sim_slab_attach: raw device addresses,
+    // e.g. of other processes' workspaces mapped through CUDA IPC)
+    struct Peer { int j0 = 0, ny = 0; void *h[2]{}, *qx[2]{}, *qy[2]{}, *zs = nullptr; uint8_t *occ = nullptr; Ctl *ctl = nullptr; } peer[8];
+    sim *group[8]{}; int ngroup = 0, grank = 0;
     cudaEvent_t ev_slab = nullptr;
     int n_inflow = 0, n_hydro = 0, n_line = 0, n_targets = 0;
     double inflow_length = 0.0;
@@ -239,9 +242,9 @@ template <typename T> FloodArgs<T> flood_args(const sim *s)
     a.dryseg = s->dry_skip ? s->dryseg : nullptr; a.dry_stride = s->dry_stride; a.nsegx = s->nsegx;
     if (s->ngroup > 1) {
         const size_t nx = (size_t)s->grid.nx;
-        const sim *lo = s->grank > 0 ? s->group[s->grank - 1] : nullptr, *hi = s->grank + 1 < s->ngroup ? s->group[s->grank + 1] : nullptr;
+        const sim::Peer *lo = s->grank > 0 ? &s->peer[s->grank - 1] : nullptr, *hi = s->grank + 1 < s->ngroup ? &s->peer[s->grank + 1] : nullptr;
         if (lo) {
-            const size_t off = (size_t)(lo->grid.ny - 1) * nx;            // its last row
+            const size_t off = (size_t)(lo->ny - 1) * nx;                  // its last row
             for (int k = 0; k < 2; ++k) { a.halo_h[0][k] = (const T *)lo->h[k] + off; a.halo_qx[0][k] = (const T *)lo->qx[k] + off; a.halo_qy[0][k] = (const T *)lo->qy[k] + off; }
             a.halo_z[0] = (const T *)lo->zs + off;
         }
@@ -290,13 +293,15 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
     a.c_exp2 = (T)(-1.4426950408889634 / p.B_s);
     // where the flood state of a cell lives: one slab (this handle's own grid) unless linked (8f-4)
     const int ng = s->ngroup > 0 ? s->ngroup : 1;
-    a.slab.n = ng; a.slab.rows = ng > 1 ? s->group[0]->grid.ny : s->gny;
+    sim::Peer self; self.j0 = s->j0; self.ny = s->grid.ny; self.zs = s->zs; self.occ = s->occ; self.ctl = s->ctl;
+    for (int k = 0; k < 2; ++k) { self.h[k] = s->h[k]; self.qx[k] = s->qx[k]; self.qy[k] = s->qy[k]; }
+    a.slab.n = ng; a.slab.rows = ng > 1 ? s->peer[0].ny : s->gny;
     for (int r = 0; r < ng; ++r) {
-        const sim *q = ng > 1 ? s->group[r] : s;
+        const sim::Peer *q = ng > 1 ? &s->peer[r] : &self;
         const ptrdiff_t off = (ptrdiff_t)q->j0 * s->grid.nx;
         for (int k = 0; k < 2; ++k) {
             a.slab.h[k][r] = (const T *)q->h[k] - off; a.slab.qx[k][r] = (const T *)q->qx[k] - off; a.slab.qy[k][r] = (const T *)q->qy[k] - off;
-            a.slab.occ[k][r] = q->occ + (size_t)k * q->ncell - off;
+            a.slab.occ[k][r] = q->occ + (size_t)k * ((size_t)q->ny * s->grid.nx) - off;
         }
     }
     a.ctl = s->ctl;
@@ -309,8 +314,11 @@ template <typename T> TailArgs<T> tail_args(const sim *s)
     a.ctl = s->ctl; a.line_cells = s->line_cells;
     {
         const int ng = s->ngroup > 0 ? s->ngroup : 1;
-        a.slab_rows = ng > 1 ? s->group[0]->grid.ny : s->gny; a.nx = s->grid.nx;
-        for (int r = 0; r < ng; ++r) { const sim *q = ng > 1 ? s->group[r] : s; a.zs_tab[r] = (T *)q->zs - (ptrdiff_t)q->j0 * s->grid.nx; }
+        a.slab_rows = ng > 1 ? s->peer[0].ny : s->gny; a.nx = s->grid.nx;
+        for (int r = 0; r < ng; ++r) {
+            void *zs = ng > 1 ? s->peer[r].zs : s->zs; const int j0 = ng > 1 ? s->peer[r].j0 : s->j0;
+            a.zs_tab[r] = (T *)zs - (ptrdiff_t)j0 * s->grid.nx;
+        }
     }
     a.n_line = s->n_line; a.bags_per_cell_layer = s->prm.bags_per_cell_layer; a.n_layers = s->prm.n_layers;
     a.layer_thickness = (T)s->prm.layer_thickness;
@@ -964,13 +972,98 @@ extern "C" int sim_slab_link(sim_t *const *h, int32_t n)
         CU(cudaStreamSynchronize(q->stream));
         drop_graphs(q);
         q->ngroup = n; q->grank = r;
-        for (int k = 0; k < n; ++k) q->group[k] = h[k];
-        if (q->flood_variant != 0 && q->flood_variant != 4) q->flood_variant = q->grid.nx % 16 == 0 ? 4 : 0;
+        for (int k = 0; k < n; ++k) {
+            q->group[k] = h[k];
+            sim::Peer &pr = q->peer[k];
+            pr.j0 = h[k]->j0; pr.ny = h[k]->grid.ny; pr.zs = h[k]->zs; pr.occ = h[k]->occ; pr.ctl = h[k]->ctl;
+            for (int b = 0; b < 2; ++b) { pr.h[b] = h[k]->h[b]; pr.qx[b] = h[k]->qx[b]; pr.qy[b] = h[k]->qy[b]; }
+        }
+        // the halo row is read by the TMA path of variant 4 (strips inside the domain) and by variant 0
+        q->flood_variant = q->grid.nx % MW == 0 && q->flood_variant != 0 ? 4 : 0;
         CU(cudaMemsetAsync(q->dryseg, 0, 2 * q->dry_stride, q->stream));
         if (!q->ev_slab) CU(cudaEventCreateWithFlags(&q->ev_slab, cudaEventDisableTiming));
         q->binned = false;
     }
     return s->grid.real_bits == 64 ? slab_refresh<double>(h, n) : slab_refresh<float>(h, n);
+}
+
+extern "C" int sim_slab_describe(sim_t *s, sim_slab_desc_t *o)
+{
+    if (!s || !o) return SIM_EINVAL;
+    std::memset(o, 0, sizeof *o);
+    o->j0 = s->j0; o->ny = s->grid.ny;
+    for (int k = 0; k < 2; ++k) { o->h[k] = (uint64_t)(uintptr_t)s->h[k]; o->qx[k] = (uint64_t)(uintptr_t)s->qx[k]; o->qy[k] = (uint64_t)(uintptr_t)s->qy[k]; }
+    o->zs = (uint64_t)(uintptr_t)s->zs; o->occ = (uint64_t)(uintptr_t)s->occ; o->ctl = (uint64_t)(uintptr_t)s->ctl;
+    o->lam_bits = (uint64_t)(uintptr_t)&s->ctl->lam_bits;
+    o->workspace = (uint64_t)(uintptr_t)s->ws; o->workspace_bytes = (uint64_t)s->ws_bytes;
+    return SIM_OK;
+}
+
+extern "C" int sim_slab_attach(sim_t *s, int32_t rank, int32_t n, const sim_slab_desc_t *d)
+{
+    if (!s || !d || n < 1 || n > MAX_SLABS || rank < 0 || rank >= n) return SIM_EINVAL;
+    DeviceGuard on_device(s);
+    if (s->ngroup) return fail(s, SIM_EINVAL, "handle is already linked");
+    if (s->prm.open_sides || s->prm.flood_order == 2 || s->prm.n_doors > 0)
+        return fail(s, SIM_EINVAL, "row slabs over processes are not combined with open edges, flood_order 2 or doors");
+    int row = 0;
+    for (int r = 0; r < n; ++r) {
+        if (d[r].j0 != row || d[r].ny <= 0) return fail(s, SIM_EINVAL, "slabs must be given in row order and cover the grid without gaps");
+        if (r + 1 < n && d[r].ny != d[0].ny) return fail(s, SIM_EINVAL, "all slabs but the last must have the same number of rows");
+        row += d[r].ny;
+    }
+    if (row != s->gny || d[rank].j0 != s->j0 || d[rank].ny != s->grid.ny) return fail(s, SIM_EINVAL, "the descriptions do not match this handle's grid");
+    if (rank > 0 && s->np > 0) return fail(s, SIM_EINVAL, "all pedestrians live on the first slab's handle");
+    CU(cudaStreamSynchronize(s->stream));
+    drop_graphs(s);
+    for (int r = 0; r < n; ++r) {
+        sim::Peer &pr = s->peer[r];
+        pr.j0 = d[r].j0; pr.ny = d[r].ny; pr.zs = (void *)(uintptr_t)d[r].zs; pr.occ = (uint8_t *)(uintptr_t)d[r].occ; pr.ctl = (Ctl *)(uintptr_t)d[r].ctl;
+        for (int b = 0; b < 2; ++b) { pr.h[b] = (void *)(uintptr_t)d[r].h[b]; pr.qx[b] = (void *)(uintptr_t)d[r].qx[b]; pr.qy[b] = (void *)(uintptr_t)d[r].qy[b]; }
+        s->group[r] = nullptr;
+    }
+    s->group[rank] = s;
+    s->ngroup = n; s->grank = rank;
+    s->flood_variant = s->grid.nx % MW == 0 && s->flood_variant != 0 ? 4 : 0;   // see sim_slab_link
+    CU(cudaMemsetAsync(s->dryseg, 0, 2 * s->dry_stride, s->stream));
+    s->binned = false;
+    return SIM_OK;
+}
+
+namespace {
+template <typename T> int slab_enqueue(sim *s, int phase)
+{
+    Marks none{nullptr, 0, s->stream};
+    if (phase == 0) {
+        if (s->np > 0) {
+            int rc = prepare_bins<T>(s);
+            if (rc != SIM_OK) return rc;
+            // pedestrian step n with the count of the next chain folded in, then that chain (it fills the N_p
+            // buffer the flood kernels of step n are not reading, in whichever slab holds the cell)
+            CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + PED_THREADS - 1) / PED_THREADS), dim3(PED_THREADS), 0, s->stream, false, ped_args_full<T>(s, 0), 1));
+            rc = enqueue_bin_chain<T>(s, s->stream, 1, none, true);
+            if (rc != SIM_OK) return rc;
+        }
+        return launch_flood<T>(s, s->stream, false);
+    }
+    if (phase == 1) { CU(launch_pdl(tail_kernel<T>, dim3(1), dim3(32), 0, s->stream, false, tail_args<T>(s), 0)); return SIM_OK; }
+    if (phase == 2) {
+        flood_chunk_flags_kernel<T><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const T *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
+        flood_lambda_kernel<T><<<592, 256, 0, s->stream>>>(flood_args<T>(s));
+        CU(cudaGetLastError());
+        return SIM_OK;
+    }
+    if (phase == 3) { tail_kernel<T><<<1, 32, 0, s->stream>>>(tail_args<T>(s), 1); CU(cudaGetLastError()); return SIM_OK; }
+    return fail(s, SIM_EINVAL, "phase must be 0..3");
+}
+}  // namespace
+
+extern "C" int sim_slab_enqueue(sim_t *s, int32_t phase)
+{
+    if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
+    if (s->ngroup < 1 || s->group[s->grank] != s) return fail(s, SIM_EINVAL, "sim_slab_attach first");
+    return DISPATCH(s, slab_enqueue, s, phase);
 }
 
 extern "C" int sim_slab_step(sim_t *const *h, int32_t n, int64_t steps)
@@ -1008,6 +1101,8 @@ extern "C" int sim_set_flood_variant(sim_t *s, int32_t variant)
     if (variant < 0 || variant > 4) return fail(s, SIM_EINVAL, "variant must be 0..4");
     if (s->prm.flood_order == 2) return fail(s, SIM_EINVAL, "flood_order = 2 has one kernel (variant 5)");
     if (s->prm.open_sides && variant != 0) return fail(s, SIM_EINVAL, "open edges are built into variants 0 and 5 only");
+    if (s->ngroup > 1 && !(variant == 0 || (variant == 4 && s->grid.nx % MW == 0)))
+        return fail(s, SIM_EINVAL, "a linked row slab runs variant 0, or variant 4 when nx is a multiple of 256 (the halo row is read by those)");
     if (variant == 4 && s->grid.nx % 16 != 0) return fail(s, SIM_EINVAL, "the TMA march kernel needs nx % 16 == 0");
     if (variant == 3 && s->grid.nx % 2 != 0) return fail(s, SIM_EINVAL, "the two-column march kernel needs nx % 2 == 0");
     if (variant == 1 && s->grid.nx % 4 != 0) return fail(s, SIM_EINVAL, "the tiled kernel needs nx % 4 == 0");

@@ -117,6 +117,8 @@ def test_link_validation():
     g = binding.SlabSim(sc, 2)
     with pytest.raises(binding.FloodpedError):
         g.sims[0].step(1)
+    with pytest.raises(binding.FloodpedError):
+        g.sims[0].set_flood_variant(4)          # 64 columns: the strip sticks out of the grid, that path reads no halo row
 
 
 def test_doors_and_trigger_on_slabs_match_the_oracle_step_by_step():
