@@ -393,6 +393,49 @@ def run_slabs(args):
                 "two runs of the SAME handle differ as well: pair forces are summed in the order of the counting sort's atomics"}))
 
 
+def run_slab_ranks(args):
+    """SURVEY 8f-4 under torchrun: ONE grid cut into WORLD_SIZE row slabs, one process and GPU per slab
+    (binding.SlabRank: CUDA-IPC peer memory, one 8-byte MAX all-reduce per step over NCCL); strong
+    scaling of the coupled step.  With --slab-backend gloo all ranks may share one GPU (how the path is
+    exercised on a single-GPU box: the reduction then goes through the host and dominates the time)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1908_05232_b200 import binding, build
+    world, rank, local = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0"))
+    dev = local % max(torch.cuda.device_count(), 1)
+    torch.cuda.set_device(dev)
+    if args.slab_backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{dev}"))
+    else:
+        dist.init_process_group("gloo")
+    if rank == 0:
+        build.build()
+    dist.barrier()
+    K, W = args.steps, max(args.warmup, 3)
+    sc = scenario(args.config)
+    g = binding.SlabRank(sc, device=f"cuda:{dev}")
+    g.step(W)
+    torch.cuda.synchronize(); dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); g.step(K); e1.record()
+    torch.cuda.synchronize(); dist.barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=f"cuda:{dev}" if args.slab_backend == "nccl" else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    st = g.sim.stats()
+    if rank == 0:
+        ncell = sc.nx * sc.ny
+        print(json.dumps({
+            "metric": "flood cell-updates/s (coupled step)", "value": ncell * K / (ms * 1e-3), "unit": "cell-updates/s",
+            "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32" if sc.real_bits == 32 else "f64", "data": "synthetic",
+            "config": {"workload": f"config{args.config}: {sc.name}", "parallelism": f"{world} row slabs, one process each ({args.slab_backend}; "
+                       f"{torch.cuda.device_count()} device(s) visible)", "flood_variant": g.sim.flood_variant()},
+            "final": {"t": st["t"], "step": st["step"]}}))
+    g.close()
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -406,7 +449,11 @@ def main():
     ap.add_argument("--march-rows", type=int, default=0, help="rows per chunk of the row-marching flood kernel (0: library default)")
     ap.add_argument("--no-overlap", action="store_true", help="pedestrian step and flood step in one chain instead of parallel graph branches")
     ap.add_argument("--slabs", type=int, default=0, help="SURVEY 8f-4: cut the grid into this many row slabs, all on cuda:0, and compare with the single handle")
+    ap.add_argument("--slab-ranks", action="store_true", help="SURVEY 8f-4 under torchrun: one grid, one row slab per rank (strong scaling) instead of one replica per rank")
+    ap.add_argument("--slab-backend", default="nccl", choices=["nccl", "gloo"], help="collective for the 8-byte wave-speed reduction of --slab-ranks")
     args = ap.parse_args()
+    if args.slab_ranks and args.impl == "ours":
+        return run_slab_ranks(args)
     if args.slabs > 1 and args.impl == "ours":
         return run_slabs(args)
     if args.impl == "reference":
