@@ -11,6 +11,7 @@
  *   (O) pedestrians per cell N_p -> roughness n = n0 (1 + min(N_p, n_cap))
  *   (F) flood cells: first-order finite-volume update of U = [h, hu, hv], Eq. (2),
  *       Riemann fluxes on hydrostatically reconstructed states, Manning friction
+ *       (sim_params_t::flood_order = 2: the second-order scheme it was reduced from)
  *   (T) t += dt ; dt for the next step from the CFL criterion, on the device
  *   (B) pedestrians binned by counting sort + prefix scan (replaces FLAMEGPU's
  *       per-cell messages)
