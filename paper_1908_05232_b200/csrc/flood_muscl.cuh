@@ -18,10 +18,11 @@
 //   phase 1  (h, qx, qy, z) of the tile + a halo of TWO cells into shared memory (z = +inf outside
 //            the domain and in solid cells: a wall);
 //   phase 2  predicted face values (4 faces x (h, qx, qy, z)) of the tile + a halo of ONE cell;
-//   phase 3  every thread: the four faces of its cell (own face value | neighbour's opposite face
-//            value, or the wall ghost), sources, finish_cell(), block-wide max of the wave speed.
+//   phase 3a every face of the tile once (left | right predicted face values, or the wall / transmissive
+//            ghost), fluxes to shared memory;
+//   phase 3b every thread: its four face fluxes, sources, finish_cell(), block-wide max of the wave speed.
 // Algorithmic bytes per cell are those of the first-order step (33 B fp32); the halo-2 re-reads
-// are L2 traffic.  Each face is evaluated by both of its cells (simple; ~2x the flux flops).
+// are L2 traffic.
 #pragma once
 
 #include "flood.cuh"
@@ -35,7 +36,9 @@ constexpr int MPX = MTX + 2, MPY = MTY + 2;            // predicted face values:
 template <typename T>
 struct MusclSmem {
     T raw[4][MRY][MRX];            // h, qx, qy, z
-    T fv[4][4][MPY][MPX];          // [face W,E,S,N][h, qx, qy, z]
+    T fv[4][4][MPY][MPX];          // predicted face values [face W,E,S,N][h, u, v, z]
+    T xf[4][MTY][MTX + 1];         // x-faces of the tile: mass flux, normal momentum as seen by the left / by the right cell, tangential
+    T yf[4][MTY + 1][MTX];         // y-faces likewise (lower / upper)
     uint8_t wet[MPY][MPX];         // cell wet at level n (h > h_dry), 2 = solid / outside
     T red[32];
 };
@@ -120,62 +123,84 @@ __global__ void __launch_bounds__(MTX * MTY) flood_muscl_kernel(FloodArgs<T> a)
                       - hdtdy * ((fqy[3] * vN - fqy[2] * vS) + a.g * T(0.5) * (fh[3] + fh[2]) * (fe[3] - fe[2]));
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
-            s.fv[f][0][py][px] = fmax(T(0), fh[f] + dh);
-            s.fv[f][1][py][px] = fqx[f] + dqx;
-            s.fv[f][2][py][px] = fqy[f] + dqy;
+            const T hp = fmax(T(0), fh[f] + dh);
+            const T r = wet ? fast_rcp(fmax(hp, a.h_dry)) : T(0);     // face velocity of a wet cell: q / max(h, h_dry); else 0
+            s.fv[f][0][py][px] = hp;
+            s.fv[f][1][py][px] = (fqx[f] + dqx) * r;
+            s.fv[f][2][py][px] = (fqy[f] + dqy) * r;
             s.fv[f][3][py][px] = fe[f] - fh[f];
         }
     }
     __syncthreads();
 
-    // phase 3: M4-M7 for my cell
+    // phase 3a: M4, every face of the tile ONCE.  x-face fx of row py lies between predicted cells (fx, py) and
+    // (fx + 1, py): the left one contributes its E face value, the right one its W face value; y-faces likewise
+    // with N | S.  A solid / outside side is the wall ghost of the other (O2.1), or, on an open domain edge, its
+    // transmissive ghost (D1).  Stored: mass flux, normal-momentum flux as seen by the left / lower and by the
+    // right / upper cell (F1 - g h*^2/2 + g h_f^2/2 with h_f that cell's own face depth), tangential flux.
+    constexpr int NXF = MTY * (MTX + 1), NYF = (MTY + 1) * MTX;
+    for (int k = tid; k < NXF + NYF; k += MTX * MTY) {
+        const bool xdir = k < NXF;
+        const int kk = xdir ? k : k - NXF;
+        const int fx = xdir ? kk % (MTX + 1) : kk % MTX, fy = xdir ? kk / (MTX + 1) : kk / MTX;
+        const int pxL = xdir ? fx : fx + 1, pyL = xdir ? fy + 1 : fy;             // left / lower cell (predicted coordinates)
+        const int pxR = xdir ? fx + 1 : fx + 1, pyR = xdir ? fy + 1 : fy + 1;
+        const int fL = xdir ? 1 : 3, fR = xdir ? 0 : 2;                           // its E | N face, the other's W | S face
+        const int wL = s.wet[pyL][pxL], wR = s.wet[pyR][pxR];
+        T f0 = T(0), FL = T(0), FR = T(0), f2 = T(0);
+        if (wL != 2 || wR != 2) {
+            T hL = s.fv[fL][0][pyL][pxL], zL = s.fv[fL][3][pyL][pxL];
+            T nL = s.fv[fL][xdir ? 1 : 2][pyL][pxL], tL = s.fv[fL][xdir ? 2 : 1][pyL][pxL];
+            T hR = s.fv[fR][0][pyR][pxR], zR = s.fv[fR][3][pyR][pxR];
+            T nR = s.fv[fR][xdir ? 1 : 2][pyR][pxR], tR = s.fv[fR][xdir ? 2 : 1][pyR][pxR];
+            const int giR = x0 + pxR - 1, gjR = y0 + pyR - 1, giL = x0 + pxL - 1, gjL = y0 + pyL - 1;   // global cells
+            bool open_out = false;
+            if (wL == 2) {                              // the right / upper cell is real
+                const bool edge = xdir ? giR == 0 : gjR == 0;
+                const bool op = edge && open_face(a, xdir ? 0 : 2, giR, gjR);
+                hL = hR; zL = zR; tL = tR; nL = op ? nR : -nR;
+                if (op) open_out = true;
+            } else if (wR == 2) {
+                const bool edge = xdir ? giL == a.nx - 1 : gjL == a.ny - 1;
+                const bool op = edge && open_face(a, xdir ? 1 : 3, giL, gjL);
+                hR = hL; zR = zL; tR = tL; nR = op ? nL : -nL;
+                if (op) open_out = true;
+            }
+            T f1L, f1R;
+            face_flux(a.g, hL, nL, tL, zL, hR, nR, tR, zR, f0, f1L, f1R, f2);
+            FL = f1L + T(0.5) * a.g * hL * hL; FR = f1R + T(0.5) * a.g * hR * hR;
+            // volume through an open face (D1): counted by the tile that owns the real cell
+            if (open_out) {
+                const bool mine = wL == 2 ? (pxR >= 1 && pxR <= MTX && pyR >= 1 && pyR <= MTY) : (pxL >= 1 && pxL <= MTX && pyL >= 1 && pyL <= MTY);
+                if (mine) add_outflow(a, dt, wL == 2 ? -f0 : f0, xdir ? a.inv_dx : a.inv_dy);
+            }
+        }
+        T *dst = xdir ? &s.xf[0][fy][fx] : &s.yf[0][fy][fx];
+        const int plane = xdir ? MTY * (MTX + 1) : (MTY + 1) * MTX;
+        dst[0] = f0; dst[plane] = FL; dst[2 * plane] = FR; dst[3 * plane] = f2;
+    }
+    __syncthreads();
+
+    // phase 3b: M5-M7 for my cell
     const int i = x0 + threadIdx.x, j = y0 + threadIdx.y;
     T lam = T(0);
     if (i < a.nx && j < a.ny) {
-        const int c = j * a.nx + i, px = threadIdx.x + 1, py = threadIdx.y + 1;
+        const int c = j * a.nx + i, tx = threadIdx.x, ty = threadIdx.y, px = tx + 1, py = ty + 1;
         T hn = T(0), qxn = T(0), qyn = T(0);
         if (s.wet[py][px] != 2) {
-            const bool wet = s.wet[py][px] == 1;
-            T F0[4], Fn[4], Ft[4], hf[4], zf[4];
-            bool open[4];
-#pragma unroll
-            for (int f = 0; f < 4; ++f) {
-                const int di = (f == 1) - (f == 0), dj = (f == 3) - (f == 2);
-                const T hi = s.fv[f][0][py][px], zi = s.fv[f][3][py][px];
-                const T ui = face_vel(wet, s.fv[f][1][py][px], hi, a.h_dry), vi = face_vel(wet, s.fv[f][2][py][px], hi, a.h_dry);
-                const T uni = f < 2 ? ui : vi, uti = f < 2 ? vi : ui;
-                T hk = hi, unk = -uni, utk = uti, zk = zi;                   // wall ghost (O2.1)
-                const int wk = s.wet[py + dj][px + di];
-                const bool edge = f == 0 ? i == 0 : f == 1 ? i == a.nx - 1 : f == 2 ? j == 0 : j == a.ny - 1;
-                open[f] = edge && open_face(a, f, i, j);
-                if (open[f]) unk = uni;                                      // transmissive ghost (D1)
-                else if (wk != 2) {
-                    const int g = f ^ 1;
-                    hk = s.fv[g][0][py + dj][px + di]; zk = s.fv[g][3][py + dj][px + di];
-                    const T uk = face_vel(wk == 1, s.fv[g][1][py + dj][px + di], hk, a.h_dry);
-                    const T vk = face_vel(wk == 1, s.fv[g][2][py + dj][px + di], hk, a.h_dry);
-                    unk = f < 2 ? uk : vk; utk = f < 2 ? vk : uk;
-                }
-                T f0, f1L, f1R, f2;
-                if (f & 1) face_flux(a.g, hi, uni, uti, zi, hk, unk, utk, zk, f0, f1L, f1R, f2);
-                else { face_flux(a.g, hk, unk, utk, zk, hi, uni, uti, zi, f0, f1R, f1L, f2); }   // f1L: as seen by my cell
-                F0[f] = f0; Fn[f] = f1L + T(0.5) * a.g * hi * hi; Ft[f] = f2;
-                hf[f] = hi; zf[f] = zi;
-            }
-            if (i == 0) F0[0] += qin * T(a.inflow[0][j]);
-            if (i == a.nx - 1) F0[1] -= qin * T(a.inflow[1][j]);
-            if (j == 0) F0[2] += qin * T(a.inflow[2][i]);
-            if (j == a.ny - 1) F0[3] -= qin * T(a.inflow[3][i]);
-            if (open[1]) add_outflow(a, dt, F0[1], a.inv_dx);
-            if (open[0]) add_outflow(a, dt, -F0[0], a.inv_dx);
-            if (open[3]) add_outflow(a, dt, F0[3], a.inv_dy);
-            if (open[2]) add_outflow(a, dt, -F0[2], a.inv_dy);
+            T FW0 = s.xf[0][ty][tx], FE0 = s.xf[0][ty][tx + 1], GS0 = s.yf[0][ty][tx], GN0 = s.yf[0][ty + 1][tx];
+            const T FnW = s.xf[2][ty][tx], FnE = s.xf[1][ty][tx + 1], FtW = s.xf[3][ty][tx], FtE = s.xf[3][ty][tx + 1];
+            const T GnS = s.yf[2][ty][tx], GnN = s.yf[1][ty + 1][tx], GtS = s.yf[3][ty][tx], GtN = s.yf[3][ty + 1][tx];
+            if (i == 0) FW0 += qin * T(a.inflow[0][j]);
+            if (i == a.nx - 1) FE0 -= qin * T(a.inflow[1][j]);
+            if (j == 0) GS0 += qin * T(a.inflow[2][i]);
+            if (j == a.ny - 1) GN0 -= qin * T(a.inflow[3][i]);
             // M5, folded into the flux differences: -dt/dx (dF - S dx)
-            const T Sx = T(0.5) * a.g * (hf[0] + hf[1]) * (zf[0] - zf[1]);
-            const T Sy = T(0.5) * a.g * (hf[2] + hf[3]) * (zf[2] - zf[3]);
+            const T Sx = T(0.5) * a.g * (s.fv[0][0][py][px] + s.fv[1][0][py][px]) * (s.fv[0][3][py][px] - s.fv[1][3][py][px]);
+            const T Sy = T(0.5) * a.g * (s.fv[2][0][py][px] + s.fv[3][0][py][px]) * (s.fv[2][3][py][px] - s.fv[3][3][py][px]);
             finish_cell(a, dt, s.raw[0][py + 1][px + 1], s.raw[1][py + 1][px + 1], s.raw[2][py + 1][px + 1],
-                        F0[1] - F0[0], (Fn[1] - Fn[0]) - Sx, Ft[1] - Ft[0],
-                        F0[3] - F0[2], Ft[3] - Ft[2], (Fn[3] - Fn[2]) - Sy,
+                        FE0 - FW0, (FnE - FnW) - Sx, FtE - FtW,
+                        GN0 - GS0, GtN - GtS, (GnN - GnS) - Sy,
                         a.n0[c], (int)OCC[c], hn, qxn, qyn, lam);
         }
         a.h[p ^ 1][c] = hn; a.qx[p ^ 1][c] = qxn; a.qy[p ^ 1][c] = qyn;
