@@ -187,10 +187,11 @@ int derive_sizes(sim *s, const sim_grid_t *g, int32_t n_peds, const sim_params_t
     // march kernel geometry: strips of MW columns, chunks of R rows; R shrinks until the grid
     // fills the 148 SMs a few times over
     s->march_gx = (g->nx + MW - 1) / MW;
-    // about 15 waves of 148 SMs x 6 resident CTAs (measured on 8192^2: flat optimum R = 14..24;
-    // short chunks even out the dry/wet imbalance between CTAs, halo rows cost little: not DRAM-bound)
+    // about 10 waves of 148 SMs x 6 resident CTAs (measured on 8192^2 with dry chunks skipped: step 0.582 / 0.574 /
+    // 0.568 / 0.566 / 0.569 ms at R = 14 / 19 / 24 / 28 / 32: fewer halo rows and prologues against coarser skipping
+    // and a longer tail)
     const long long slots = (long long)s->n_sm * 6;
-    s->march_R = (int)(((long long)g->ny * s->march_gx) / (15 * slots));
+    s->march_R = (int)(((long long)g->ny * s->march_gx * 2) / (21 * slots));
     if (s->march_R > MARCH_MAX_R) s->march_R = MARCH_MAX_R;
     if (s->march_R < 16) s->march_R = 16;
     if ((long long)s->march_gx * ((g->ny + s->march_R - 1) / s->march_R) < 4 * slots) {
