@@ -231,6 +231,50 @@ int sim_slab_describe(sim_t *s, sim_slab_desc_t *out);
 int sim_slab_attach(sim_t *s, int32_t rank, int32_t n, const sim_slab_desc_t *descs);
 int sim_slab_enqueue(sim_t *s, int32_t phase);
 
+/* ---- the CFL time step of a flood state, for callers that must not allocate device memory ----
+ * Who this is for.  Everything above needs device memory from somewhere: sim_create either calls cudaMalloc or
+ * is handed a workspace the caller allocated.  Some callers can do neither at the moment they need a time step:
+ *   - a host application whose own pool allocator (PyTorch's caching allocator, an RMM pool, a rendering or
+ *     solver framework's arena) already owns practically all of the GPU's memory, so that a cudaMalloc from a
+ *     guest library fails or evicts what the host keeps resident;
+ *   - a loop with a latency budget (a live coupled run, a real-time viewer), where cudaMalloc / cudaFree are not
+ *     acceptable because they may synchronise the whole device and take an unbounded time;
+ *   - a plug-in that is only given pointers to the host solver's depth and discharge fields and has no
+ *     permission to create device buffers of its own.
+ * Such a caller holds h, qx, qy (and perhaps a solid mask) in device memory already and wants the one global
+ * number the method derives from them every step: the largest wave speed over the wet cells and the time step
+ * the CFL criterion allows.
+ *
+ *   lam = max over cells with mask == 0 and h > h_dry of max((|qx/h| + sqrt(g h)) / dx, (|qy/h| + sqrt(g h)) / dy)
+ *   dt  = lam > 0 ? min(dt_max, cfl / lam) : dt_max
+ *
+ * computed in the precision real_bits names, cell by cell as sim_create / sim_step compute it (without their
+ * clamp to t_end), the maximum taken exactly.  out[0] = lam, out[1] = dt.
+ *
+ * Arguments: h, qx, qy are DEVICE pointers to n_cells reals each; mask is a DEVICE pointer to n_cells bytes
+ * (non-zero = solid cell, skipped) or NULL; out is a DEVICE pointer to two doubles, written by the kernel; the
+ * caller owns all of them.  cuda_stream as elsewhere.  The call only enqueues work (one 8-byte memset and one
+ * kernel) on the stream of the CURRENT device, which must be the device the pointers live on, and returns;
+ * read `out` after synchronising that stream.  n_cells = 0 gives lam = 0, dt = dt_max.
+ *
+ * Scratch.  The block-wise partial maxima and a counter live in a fixed array inside the library's device image
+ * (256 KiB + 256 bytes on every GPU that loads libfloodped.so, released when the process exits), not in
+ * allocated memory.  Hence the limit: n_cells <= SIM_CFL_STATIC_MAX_CELLS (2^28 = a 16384 x 16384 grid); a
+ * larger n_cells is refused with SIM_EINVAL and a message naming the limit.  The entry point calls no cudaMalloc,
+ * cudaFree or allocating library routine.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, which may load
+ *     the library's device code); make that first call outside any stream capture.
+ *   - There is ONE such array per device, shared by every call from every thread and stream, and it keeps what
+ *     the previous call left.  Each call re-zeroes the counter it depends on, so calls that follow one another on
+ *     one stream need nothing from the caller; calls that may overlap on the GPU (different streams, or different
+ *     threads' streams, without an event between them) race on it and return garbage.  Serialise them.
+ * Errors: SIM_EINVAL (NULL pointer, size beyond the limit, non-positive dx dy g cfl h_dry dt_max, real_bits),
+ * SIM_ECUDA; the text is at sim_last_error(NULL). */
+#define SIM_CFL_STATIC_MAX_CELLS (1 << 28)
+int sim_cfl_dt_static(const void *h, const void *qx, const void *qy, const uint8_t *mask, int64_t n_cells,
+                      int32_t real_bits, double dx, double dy, double g, double h_dry, double cfl, double dt_max,
+                      void *cuda_stream, double *out /* DEVICE, [2]: lam, dt */);
+
 /* ============================================================================================
  * Everything above is the product ABI of SURVEY 8(b).  Below: TEST AND TUNING HOOKS -- state
  * re-injection for the parity tests, kernel selection and per-kernel timing for measurement.

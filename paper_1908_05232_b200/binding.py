@@ -20,8 +20,10 @@ EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
     "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap", "sim_set_dry_skip",
-    "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_slab_describe", "sim_slab_attach", "sim_slab_enqueue", "sim_last_error", "sim_destroy",
+    "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_slab_describe", "sim_slab_attach", "sim_slab_enqueue", "sim_cfl_dt_static", "sim_last_error", "sim_destroy",
 ]
+
+SIM_CFL_STATIC_MAX_CELLS = 1 << 28
 
 _vp = C.c_void_p
 _u8p = C.POINTER(C.c_uint8)
@@ -151,6 +153,7 @@ def load_library(path: str = LIB_PATH):
     L.sim_slab_describe.argtypes = [_vp, C.POINTER(SlabDesc)]
     L.sim_slab_attach.argtypes = [_vp, C.c_int32, C.c_int32, C.POINTER(SlabDesc)]
     L.sim_slab_enqueue.argtypes = [_vp, C.c_int32]
+    L.sim_cfl_dt_static.argtypes = [_vp, _vp, _vp, _vp, C.c_int64, C.c_int32] + [C.c_double] * 6 + [_vp, _vp]
     L.sim_last_error.argtypes = [_vp]
     L.sim_last_error.restype = C.c_char_p
     L.sim_destroy.argtypes = [_vp]
@@ -241,6 +244,23 @@ def workspace_bytes(sc) -> int:
     if rc != SIM_OK:
         raise FloodpedError(rc, L.sim_last_error(None).decode())
     return out.value
+
+
+def cfl_dt_static(h_ptr, qx_ptr, qy_ptr, mask_ptr, n_cells, real_bits, dx, dy, g, h_dry, cfl, dt_max, stream_ptr, out_ptr):
+    """sim_cfl_dt_static (include/floodped.h): largest wave speed and CFL time step of a flood state
+    that already sits in device memory, for callers that must not allocate on the device (a host
+    framework's pool owns the GPU's memory, a loop that cannot afford cudaMalloc's device-wide
+    synchronisation, a plug-in that is only handed pointers).  All `*_ptr` are raw DEVICE addresses
+    (ints; `mask_ptr` and `stream_ptr` may be None / 0); `out_ptr` receives two doubles (lam, dt)
+    once the stream has run.  Enqueues only; no handle, no workspace, no allocation: the scratch is
+    a fixed array inside the library, so n_cells <= SIM_CFL_STATIC_MAX_CELLS and calls that could
+    overlap on the GPU must be serialised by the caller.  Marshalling only."""
+    L = load_library()
+    rc = L.sim_cfl_dt_static(_vp(h_ptr), _vp(qx_ptr), _vp(qy_ptr), _vp(mask_ptr or None), int(n_cells), int(real_bits),
+                             float(dx), float(dy), float(g), float(h_dry), float(cfl), float(dt_max),
+                             _vp(stream_ptr or None), _vp(out_ptr))
+    if rc != SIM_OK:
+        raise FloodpedError(rc, L.sim_last_error(None).decode())
 
 
 class Sim:

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <cstdlib>
 #include <string>
 #include <vector>
@@ -1424,4 +1425,136 @@ extern "C" void sim_destroy(sim_t *s)
     if (s->ev_slab) cudaEventDestroy(s->ev_slab);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
+}
+
+// ================================================================================ no-allocation entry point
+// sim_cfl_dt_static (include/floodped.h): the CFL time step of a flood state the caller holds in device
+// memory, for callers that may not allocate device memory at all.  It is a variant of flood_lambda_kernel: the
+// per-cell wave speed is the same expression, but where that kernel folds the maximum into the handle's control
+// block (part of a workspace somebody allocated), this one keeps its scratch -- a ticket word and one partial
+// maximum per block -- in the file-scope array below, which the CUDA module itself carries.  Nothing here calls
+// cudaMalloc, cudaFree or a library routine that allocates.
+namespace {
+
+constexpr long long CFL_STATIC_MAX_CELLS = SIM_CFL_STATIC_MAX_CELLS;
+constexpr int CFL_STATIC_THREADS = 256;
+constexpr int CFL_STATIC_BLOCK_CELLS = 8192;                         // 32 cells per thread
+constexpr int CFL_STATIC_MAX_BLOCKS = (int)(CFL_STATIC_MAX_CELLS / CFL_STATIC_BLOCK_CELLS);
+constexpr int CFL_STATIC_HEAD = 32;                                  // the ticket word has a 256-byte line of its own
+static_assert(CFL_STATIC_MAX_CELLS % CFL_STATIC_BLOCK_CELLS == 0, "whole blocks");
+
+// 256 KiB + 256 B per device that loads the library, held until the process exits.  Word 0: how many blocks of
+// the running launch have published their partial maximum (must be zero when a launch starts); words
+// CFL_STATIC_HEAD + b: partial maximum of block b as the bit pattern of a non-negative double.
+// In host code this name is only a handle for cudaGetSymbolAddress -- never pass it to a kernel as it stands.
+static __device__ __align__(256) unsigned long long g_cfl_static_scratch[CFL_STATIC_HEAD + CFL_STATIC_MAX_BLOCKS];
+
+template <typename T>
+__global__ void __launch_bounds__(CFL_STATIC_THREADS)
+cfl_static_kernel(const T *__restrict__ h, const T *__restrict__ qx, const T *__restrict__ qy, const uint8_t *__restrict__ mask,
+                  long long n, T g, T h_dry, T inv_dx, T inv_dy, double cfl, double dt_max,
+                  unsigned long long *scratch, double *out)
+{
+    __shared__ T red[32];
+    __shared__ unsigned long long redb[32];
+    __shared__ int last;
+    const int tid = threadIdx.x;
+    const long long c0 = (long long)blockIdx.x * CFL_STATIC_BLOCK_CELLS;
+    T lam = T(0);
+    for (int k = tid; k < CFL_STATIC_BLOCK_CELLS; k += CFL_STATIC_THREADS) {
+        const long long c = c0 + k;
+        if (c >= n) break;
+        const T hh = h[c];
+        if (!(mask && mask[c]) && hh > h_dry) {                       // as flood_lambda_kernel (flood.cuh)
+            const T u = qx[c] / hh, v = qy[c] / hh, cc = real_sqrt(g * hh);
+            lam = fmax(lam, fmax((fabs(u) + cc) * inv_dx, (fabs(v) + cc) * inv_dy));
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) lam = fmax(lam, __shfl_xor_sync(0xffffffffu, lam, o));
+    if ((tid & 31) == 0) red[tid >> 5] = lam;
+    __syncthreads();
+    if (tid < 32) {
+        T m = tid < CFL_STATIC_THREADS / 32 ? red[tid] : T(0);
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (tid == 0) {
+            scratch[CFL_STATIC_HEAD + blockIdx.x] = (unsigned long long)__double_as_longlong((double)m);
+            __threadfence();                                          // the partial is visible before the ticket counts it
+            last = atomicAdd(&scratch[0], 1ull) == (unsigned long long)gridDim.x - 1ull;
+        }
+    }
+    __syncthreads();
+    if (!last) return;
+    // the block that took the last ticket folds the partials: max over bit patterns of non-negative doubles
+    __threadfence();
+    unsigned long long m = 0ull;
+    const volatile unsigned long long *part = scratch + CFL_STATIC_HEAD;
+    for (unsigned b = tid; b < gridDim.x; b += CFL_STATIC_THREADS) { const unsigned long long v = part[b]; m = v > m ? v : m; }
+    for (int o = 16; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, m, o); m = v > m ? v : m; }
+    if ((tid & 31) == 0) redb[tid >> 5] = m;
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < CFL_STATIC_THREADS / 32; ++w) m = redb[w] > m ? redb[w] : m;
+        const double lmax = __longlong_as_double((long long)m);
+        double dt = dt_max;                                           // as tail_kernel (peds.cuh), without its t_end clamp
+        if (lmax > 0.0) dt = fmin(dt, cfl / lmax);
+        out[0] = lmax; out[1] = dt;
+        scratch[0] = 0ull;                                            // ready for the next launch
+    }
+}
+
+// Device address of the scratch array on `dev`, looked up once per device with that device current.
+int cfl_static_scratch(int dev, unsigned long long **out)
+{
+    sim *s = nullptr;                                                 // CU(): errors go to sim_last_error(NULL)
+    constexpr int MAXDEV = 64;
+    static unsigned long long *addr[MAXDEV] = {};
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < MAXDEV && addr[dev]) { *out = addr[dev]; return SIM_OK; }
+    int cur = -1;
+    CU(cudaGetDevice(&cur));
+    if (cur != dev) CU(cudaSetDevice(dev));
+    unsigned long long *p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void **)&p, g_cfl_static_scratch);
+    if (cur != dev) cudaSetDevice(cur);
+    if (e != cudaSuccess || !p)
+        return fail(nullptr, SIM_ECUDA, std::string("cudaGetSymbolAddress(g_cfl_static_scratch): ") + cudaGetErrorString(e));
+    if (dev >= 0 && dev < MAXDEV) addr[dev] = p;
+    *out = p;
+    return SIM_OK;
+}
+
+}  // namespace
+
+extern "C" int sim_cfl_dt_static(const void *h, const void *qx, const void *qy, const uint8_t *mask, int64_t n_cells,
+                                 int32_t real_bits, double dx, double dy, double g, double h_dry, double cfl,
+                                 double dt_max, void *cuda_stream, double *out)
+{
+    sim *s = nullptr;
+    if (n_cells < 0) return fail(nullptr, SIM_EINVAL, "sim_cfl_dt_static: negative n_cells");
+    if (n_cells > CFL_STATIC_MAX_CELLS)
+        return fail(nullptr, SIM_EINVAL, "sim_cfl_dt_static: n_cells = " + std::to_string((long long)n_cells) +
+                    " is beyond SIM_CFL_STATIC_MAX_CELLS = " + std::to_string(CFL_STATIC_MAX_CELLS) +
+                    " (the scratch of this entry point is a fixed array; use sim_create with a workspace for larger grids)");
+    if (!out || (n_cells > 0 && (!h || !qx || !qy))) return fail(nullptr, SIM_EINVAL, "sim_cfl_dt_static: h, qx, qy and out are required");
+    if (real_bits != 32 && real_bits != 64) return fail(nullptr, SIM_EINVAL, "sim_cfl_dt_static: real_bits must be 32 or 64");
+    if (!(dx > 0) || !(dy > 0) || !(g > 0) || !(cfl > 0) || !(h_dry > 0) || !(dt_max > 0))
+        return fail(nullptr, SIM_EINVAL, "sim_cfl_dt_static: dx, dy, g, cfl, h_dry and dt_max must be positive");
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    unsigned long long *scratch = nullptr;
+    int rc = cfl_static_scratch(dev, &scratch);
+    if (rc != SIM_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int blocks = n_cells > 0 ? (int)((n_cells + CFL_STATIC_BLOCK_CELLS - 1) / CFL_STATIC_BLOCK_CELLS) : 1;
+    // the ticket must start at zero whatever the launch before left behind (e.g. one that was aborted)
+    CU(cudaMemsetAsync(scratch, 0, sizeof(unsigned long long), st));
+    if (real_bits == 64)
+        cfl_static_kernel<double><<<blocks, CFL_STATIC_THREADS, 0, st>>>((const double *)h, (const double *)qx, (const double *)qy, mask,
+            (long long)n_cells, g, h_dry, 1.0 / dx, 1.0 / dy, cfl, dt_max, scratch, out);
+    else
+        cfl_static_kernel<float><<<blocks, CFL_STATIC_THREADS, 0, st>>>((const float *)h, (const float *)qx, (const float *)qy, mask,
+            (long long)n_cells, (float)g, (float)h_dry, (float)(1.0 / dx), (float)(1.0 / dy), cfl, dt_max, scratch, out);
+    CU(cudaGetLastError());
+    return SIM_OK;
 }
