@@ -218,9 +218,15 @@ int sim_slab_step(sim_t *const *handles, int32_t n, int64_t steps);
  *     all-reduce MAX over the ranks of the 8 bytes at `lam_bits` (NCCL; it is also the only barrier
  *                              the step needs: every peer access of step n is ordered before it)
  *     sim_slab_enqueue(s, 1)   tail: t += dt, next dt from the global wave speed
- * and after attaching, once: sim_slab_enqueue(s, 2) (wave speed of the initial state), the same
- * all-reduce, sim_slab_enqueue(s, 3).  No doors in this mode (newcomers are placed by the tail, after
- * the binning chain has run). */
+ * and after attaching, once: sim_slab_enqueue(s, 2) (the pedestrians binned and counted into the N_p
+ * of whichever slab holds their cell, wave speed of the initial state), the same all-reduce,
+ * sim_slab_enqueue(s, 3).  The same three calls, on every rank, after anything that invalidates the
+ * bins (sim_write_peds, sim_set_deterministic, ...): phase 0 fails with SIM_EINVAL otherwise, because
+ * bins made inside phase 0 would put N_p into another process's slab while its flood kernel reads it.  No doors in this mode (newcomers are placed by the tail, after
+ * the binning chain has run).  One peer access comes AFTER the all-reduce: the tail of the first slab
+ * raises the bed where responders have dropped sandbags, and nothing orders that write
+ * against another process's next flood kernel.  sim_slab_attach therefore fails with SIM_EINVAL
+ * unless every barrier cell lies in the first slab's rows; sim_slab_link has no such limit. */
 typedef struct {
     int32_t  j0, ny;                            /* rows [j0, j0 + ny) of the grid                     */
     uint64_t h[2], qx[2], qy[2], zs, occ, ctl;  /* device addresses of the slab's arrays              */
@@ -320,6 +326,18 @@ int sim_set_overlap(sim_t *s, int32_t on);
  * zeros (dry ground: every flux is zero, the result is zeros), reading and writing nothing for them;
  * 0: every chunk is computed.  Same results bit for bit. */
 int sim_set_dry_skip(sim_t *s, int32_t on);
+/* Reproducible pedestrian results (the GPU model "reproduced the same predictions as the
+ * sequential counterpart"; SURVEY 8a-B "stable-enough scatter").
+ * 0 (default): the slot an agent takes inside its sort bin is the order in which warps reach an
+ * atomic counter; the social force is summed in slot order, so two runs of the same
+ * input differ in the last bits of every agent that has neighbours, and a crowd at an exit
+ * amplifies that within a few hundred steps.
+ * 1: two more kernels per step order every bin by ORIGINAL agent id (O(agents per bin) per agent):
+ * the forces are summed bin by bin in increasing id -- the order of the oracle's cell lists -- and
+ * the results are the same bits on every run, on any number of row slabs, and in whatever order the
+ * agents were written.  Inactive slots (behind the last bin) keep their arrival order.
+ * Takes effect from the next step; the flood kernels are deterministic either way. */
+int sim_set_deterministic(sim_t *s, int32_t on);
 /* Number of kernels sim_step launches per coupled step (for launch accounting). */
 int sim_kernels_per_step(const sim_t *s);
 

@@ -19,7 +19,7 @@ SIM_OK, SIM_EINVAL, SIM_ENOMEM, SIM_ECUDA, SIM_ENOTFINITE = 0, -1, -2, -3, -4
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_step", "sim_step_profiled", "sim_read_flood", "sim_read_conserved",
     "sim_read_occupancy", "sim_read_peds", "sim_get_stats", "sim_bin_peds", "sim_write_flood",
-    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap", "sim_set_dry_skip",
+    "sim_write_peds", "sim_set_time", "sim_set_barrier", "sim_test_philox", "sim_set_flood_variant", "sim_get_flood_variant", "sim_set_march_rows", "sim_set_overlap", "sim_set_dry_skip", "sim_set_deterministic",
     "sim_kernels_per_step", "sim_slab_link", "sim_slab_step", "sim_slab_describe", "sim_slab_attach", "sim_slab_enqueue", "sim_cfl_dt_static", "sim_last_error", "sim_destroy",
 ]
 
@@ -147,6 +147,7 @@ def load_library(path: str = LIB_PATH):
     L.sim_set_march_rows.argtypes = [_vp, C.c_int32]
     L.sim_set_overlap.argtypes = [_vp, C.c_int32]
     L.sim_set_dry_skip.argtypes = [_vp, C.c_int32]
+    L.sim_set_deterministic.argtypes = [_vp, C.c_int32]
     L.sim_kernels_per_step.argtypes = [_vp]
     L.sim_slab_link.argtypes = [C.POINTER(_vp), C.c_int32]
     L.sim_slab_step.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int64]
@@ -337,6 +338,10 @@ class Sim:
     def set_dry_skip(self, on):
         self._chk(self._L.sim_set_dry_skip(self._h, int(bool(on))))
 
+    def set_deterministic(self, on):
+        """Bins ordered by original agent id: same bits on every run (include/floodped.h)."""
+        self._chk(self._L.sim_set_deterministic(self._h, int(bool(on))))
+
     def flood_variant(self) -> int:
         return self._L.sim_get_flood_variant(self._h)
 
@@ -505,7 +510,17 @@ class SlabRank:
         self._lam = ws[off:off + 8].view(torch.int64)      # bit pattern of a non-negative double: ordered like an integer
         self._nccl = dist.get_backend() == "nccl"
         dist.barrier()
+        self.resync()
+
+    def resync(self):
+        """(re)make the bins and N_p of the state in place and the time step from the global wave speed;
+        collective: every rank calls it, after attaching and after any change of pedestrians or modes"""
         self._phase(2); self._reduce(); self._phase(3)
+
+    def set_deterministic(self, on):
+        """collective: sim_set_deterministic on this rank's handle, then resync()"""
+        self.sim.set_deterministic(on)
+        self.resync()
 
     def _phase(self, k):
         self.sim._chk(self._L.sim_slab_enqueue(self.sim._h, int(k)))

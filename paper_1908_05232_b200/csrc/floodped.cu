@@ -60,12 +60,14 @@ struct sim {
     void *h[2]{}, *qx[2]{}, *qy[2]{}, *zs = nullptr, *z0 = nullptr, *n0 = nullptr, *scratch_real[3]{};
     uint8_t *occ = nullptr, *mask = nullptr, *inflow[4]{}, *nav = nullptr;
     int32_t *line_cells = nullptr;
+    int line_row_max = -1;           // highest grid row that holds a barrier cell (host copy for sim_slab_attach)
     double *hydro_t = nullptr, *hydro_q = nullptr;
     struct { void *x, *y, *vx, *vy, *vpref, *timer; uint8_t *role, *fsm, *state, *active; int32_t *id, *cell; } P[2]{};
     void *ped_out[5]{};             // gather targets (x y vx vy timer) in original order
     uint8_t *ped_out_u8[3]{};
     int32_t *ped_out_i32[2]{};
     int32_t *key = nullptr, *off = nullptr, *count = nullptr, *start = nullptr, *cellprev = nullptr;
+    int32_t *perm = nullptr; int deterministic = 0;       // sim_set_deterministic: bins ordered by original id
     void *bxy = nullptr;              // (x, y) of the sorted level-n agents, interleaved, for the pair loop
     unsigned long long *scan_status = nullptr;
     Ctl *ctl = nullptr;
@@ -147,6 +149,7 @@ size_t layout(sim *s, Bump &b)
     for (int k = 0; k < 3; ++k) s->ped_out_u8[k] = b.take<uint8_t>(np);
     for (int k = 0; k < 2; ++k) s->ped_out_i32[k] = b.take<int32_t>(np);
     s->key = b.take<int32_t>(np); s->off = b.take<int32_t>(np); s->cellprev = b.take<int32_t>(2 * np);
+    s->perm = b.take<int32_t>(np);
     s->bxy = real(2 * (size_t)np);
     s->count = b.take<int32_t>((size_t)s->nbins + 2); s->start = b.take<int32_t>((size_t)s->nbins + 3);
     s->ghost_zero = b.take<double>(MW); s->ghost_inf = b.take<double>(MW);
@@ -287,7 +290,7 @@ template <typename T> PedArgs<T> ped_args(const sim *s)
     a.drop_i = p.drop_cell % s->grid.nx; a.drop_j = p.drop_cell / s->grid.nx;
     a.arrive = p.arrive_cells;
     a.A = ped_soa<T>(s, 0); a.B = ped_soa<T>(s, 1);
-    a.key = s->key; a.off = s->off; a.count = s->count; a.start = s->start; a.cellprev = s->cellprev;
+    a.key = s->key; a.off = s->off; a.perm = s->perm; a.count = s->count; a.start = s->start; a.cellprev = s->cellprev;
     a.mask = s->mask; a.nav = s->nav;
     a.cellprev_stride = (size_t)s->np; a.pipelined = 0;
     a.bxy = (VecN<T, 2> *)s->bxy;
@@ -316,7 +319,7 @@ template <typename T> TailArgs<T> tail_args(const sim *s)
     a.ctl = s->ctl; a.line_cells = s->line_cells;
     {
         const int ng = s->ngroup > 0 ? s->ngroup : 1;
-        a.slab_rows = ng > 1 ? s->peer[0].ny : s->gny; a.nx = s->grid.nx;
+        a.slab_rows = ng > 1 ? s->peer[0].ny : s->gny; a.nx = s->grid.nx; a.n_slabs = ng;
         for (int r = 0; r < ng; ++r) {
             void *zs = ng > 1 ? s->peer[r].zs : s->zs; const int j0 = ng > 1 ? s->peer[r].j0 : s->j0;
             a.zs_tab[r] = (T *)zs - (ptrdiff_t)j0 * s->grid.nx;
@@ -371,6 +374,10 @@ template <typename T> int enqueue_bin_chain(sim *s, cudaStream_t st, int pipelin
     mark();
     CU(launch_pdl(scan_bins_kernel, dim3((n_items + SCAN_TILE - 1) / SCAN_TILE), dim3(SCAN_THREADS), 0, st, pdl,
                   s->count, s->start, n_items, s->scan_status, s->ctl, pipelined, pa.pdl_early));
+    if (s->deterministic) {                           // bins ordered by original id (see ped_rank_kernel)
+        CU(launch_pdl(ped_perm_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
+        CU(launch_pdl(ped_rank_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
+    }
     mark();
     CU(launch_pdl(ped_scatter_kernel<T>, dim3(nb), dim3(256), 0, st, pdl, pa));
     mark();
@@ -704,6 +711,7 @@ extern "C" int sim_create(const sim_grid_t *grid, const sim_topo_t *topo, const 
     for (int k = 0; k < p->n_line; ++k) {
         if (!cell_ok(p->line_cells[k])) return bail(fail(s, SIM_EINVAL, "barrier cell out of range"));
         if (topo->mask && topo->mask[p->line_cells[k]]) return bail(fail(s, SIM_EINVAL, "barrier cell is solid"));
+        s->line_row_max = std::max(s->line_row_max, p->line_cells[k] / nx);
     }
     if (p->n_line > 0 && p->n_layers > 0 && p->bags_per_cell_layer < 1)
         return bail(fail(s, SIM_EINVAL, "bags_per_cell_layer must be >= 1"));
@@ -827,7 +835,7 @@ extern "C" int sim_step_profiled(sim_t *s, int64_t n, double *kernel_ms)
     return DISPATCH(s, step_profiled, s, n, kernel_ms);
 }
 
-extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? (s->overlap ? 6 : 7) - (s->np < 65536 ? 1 : 0) : 2) : 0; }
+extern "C" int sim_kernels_per_step(const sim_t *s) { return s ? (s->np > 0 ? (s->overlap ? 6 : 7) - (s->np < 65536 ? 1 : 0) + (s->deterministic ? 2 : 0) : 2) : 0; }
 
 extern "C" int sim_set_march_rows(sim_t *s, int32_t rows)
 {
@@ -1016,6 +1024,12 @@ extern "C" int sim_slab_attach(sim_t *s, int32_t rank, int32_t n, const sim_slab
     }
     if (row != s->gny || d[rank].j0 != s->j0 || d[rank].ny != s->grid.ny) return fail(s, SIM_EINVAL, "the descriptions do not match this handle's grid");
     if (rank > 0 && s->np > 0) return fail(s, SIM_EINVAL, "all pedestrians live on the first slab's handle");
+    // A sandbag deposit raises the bed from the FIRST slab's tail kernel (the pedestrians live there).  Into
+    // another process's rows that write is not ordered against that process's next flood kernel: the one
+    // exchange of the step, the wave-speed all-reduce, comes before the tails.  So the line must lie in
+    // the first slab's rows (sim_slab_link, one process and one host thread launching everything, has no such limit).
+    if (n > 1 && s->n_line > 0 && s->line_row_max >= d[0].ny)
+        return fail(s, SIM_EINVAL, "row slabs over processes: every barrier cell must lie in the first slab's rows");
     CU(cudaStreamSynchronize(s->stream));
     drop_graphs(s);
     for (int r = 0; r < n; ++r) {
@@ -1038,8 +1052,10 @@ template <typename T> int slab_enqueue(sim *s, int phase)
     Marks none{nullptr, 0, s->stream};
     if (phase == 0) {
         if (s->np > 0) {
-            int rc = prepare_bins<T>(s);
-            if (rc != SIM_OK) return rc;
+            // The bins (and the N_p they put into the OTHER processes' slabs) must be in place before any
+            // rank's flood kernel of this step starts: only phase 2 has the all-reduce between it and them.
+            if (!s->binned) return fail(s, SIM_EINVAL, "pedestrians or modes changed since the bins were made: run phase 2, the all-reduce and phase 3 again (binding.SlabRank.resync)");
+            int rc = SIM_OK;
             // pedestrian step n with the count of the next chain folded in, then that chain (it fills the N_p
             // buffer the flood kernels of step n are not reading, in whichever slab holds the cell)
             CU(launch_pdl(ped_step_kernel<T>, dim3((s->np + PED_THREADS - 1) / PED_THREADS), dim3(PED_THREADS), 0, s->stream, false, ped_args_full<T>(s, 0), 1));
@@ -1050,6 +1066,11 @@ template <typename T> int slab_enqueue(sim *s, int phase)
     }
     if (phase == 1) { CU(launch_pdl(tail_kernel<T>, dim3(1), dim3(32), 0, s->stream, false, tail_args<T>(s), 0)); return SIM_OK; }
     if (phase == 2) {
+        if (s->np > 0) {                               // binning chain of the first step: its N_p lands in every slab before the all-reduce
+            s->binned = false;
+            int rc = prepare_bins<T>(s);
+            if (rc != SIM_OK) return rc;
+        }
         flood_chunk_flags_kernel<T><<<dim3(s->march_gx, s->march_gy), 256, 0, s->stream>>>((const T *)s->zs, s->grid.nx, s->grid.ny, s->march_R, s->chunk_flag);
         flood_lambda_kernel<T><<<592, 256, 0, s->stream>>>(flood_args<T>(s));
         CU(cudaGetLastError());
@@ -1123,6 +1144,17 @@ extern "C" int sim_set_dry_skip(sim_t *s, int32_t on)
     s->dry_skip = on ? 1 : 0;
     drop_graphs(s);
     CU(cudaMemsetAsync(s->dryseg, 0, 2 * s->dry_stride, s->stream));
+    return SIM_OK;
+}
+
+extern "C" int sim_set_deterministic(sim_t *s, int32_t on)
+{
+    if (!s) return SIM_EINVAL;
+    DeviceGuard on_device(s);
+    CU(cudaStreamSynchronize(s->stream));
+    s->deterministic = on ? 1 : 0;
+    s->binned = false;                     // the bins in place were ordered the other way: sort again before the next step
+    drop_graphs(s);
     return SIM_OK;
 }
 
@@ -1210,6 +1242,7 @@ template <typename T> int bin_peds_t(sim *s, int32_t *key, int32_t *order, int32
         if (halt) { c.halt = 0; CU(cudaMemcpyAsync(s->ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream)); }
         ped_bin_count_kernel<T><<<nb, 256, 0, s->stream>>>(pa, 0);
         scan_bins_kernel<<<(n_items + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, s->stream>>>(s->count, s->start, n_items, s->scan_status, s->ctl, 0, 0);
+        if (s->deterministic) { ped_perm_kernel<T><<<nb, 256, 0, s->stream>>>(pa); ped_rank_kernel<T><<<nb, 256, 0, s->stream>>>(pa); }
         ped_scatter_kernel<T><<<nb, 256, 0, s->stream>>>(pa);
         ped_key_by_id_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 0), s->key, np, s->ped_out_i32[0]);
         ped_gather_kernel<T><<<nb, 256, 0, s->stream>>>(ped_soa<T>(s, 1), np, s->grid.nx, (T)1, (T)1, s->gny,

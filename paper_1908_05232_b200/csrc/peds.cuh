@@ -47,6 +47,7 @@ struct PedArgs {
     VecN<T, 2> *bxy;                 // (x, y) of B interleaved: one 64/128-bit load per candidate
     T c_exp1, c_exp2;                // fp32 pair force: A_s e^{(2r-d)/B_s} = 2^{c_exp1 + c_exp2 d}
     int32_t *key, *off;              // per slot of A: bin key, rank inside the bin
+    int32_t *perm;                   // deterministic mode only: [n] sorted slot -> slot of A (ped_perm_kernel)
     int32_t *count;                  // [nbins+1] (zeroed by the scan after use)
     int32_t *start;                  // [nbins+2] exclusive scan
     // N_p per cell is double-buffered by flood parity: the binning chain of step n+1 runs beside the
@@ -228,6 +229,48 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_bins_kernel(int32_t *count,
     }
 }
 
+// ---------------------------------------------------------------------------------- (B) order
+// Deterministic mode (sim_set_deterministic).  The rank an agent takes inside its bin above is the
+// return value of an atomicAdd, i.e. the order in which warps happened to arrive: the sorted buffer
+// is a valid counting sort, but which slot of its bin an agent lands in differs from run to run,
+// and the pair loop sums the forces in slot order, so the last bits of every agent in a
+// crowd differ too.  These two kernels, run between the scan and the scatter, replace that rank by
+// the agent's rank BY ORIGINAL ID among the agents of its bin: the sorted order becomes a pure
+// function of the (id, position) set -- the same on every run, for any number of row slabs and
+// whatever order the agents were handed over in -- and it is the order in which the oracle walks
+// its cell lists (increasing agent index per bin).
+//   ped_perm_kernel : perm[start[key] + atomic rank] = slot of A  (which agents share a bin)
+//   ped_rank_kernel : one thread per sorted slot counts the ids of its bin below its own: O(k) per
+//                     agent, k = agents per bin (a handful on Configs 1-4, about 30 on Config 5).
+// The slots past the last bin (inactive agents, key = nbins) keep their arrival order: nothing but
+// the order output of sim_bin_peds reads them by slot, and there may be 10^6 of them.
+template <typename T>
+__global__ void __launch_bounds__(256) ped_perm_kernel(PedArgs<T> a)
+{
+    if (a.pdl_early) pdl_trigger();
+    pdl_wait();
+    if (chain_sel(a) < 0) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= a.n) return;
+    a.perm[a.start[a.key[s]] + a.off[s]] = s;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) ped_rank_kernel(PedArgs<T> a)
+{
+    if (a.pdl_early) pdl_trigger();
+    pdl_wait();
+    if (chain_sel(a) < 0) return;
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d >= a.n) return;
+    const int s = a.perm[d], b = a.key[s];
+    if (b >= a.nbins) return;
+    const int id = a.A.id[s];
+    int below = 0;
+    for (int j = a.start[b]; j < a.start[b + 1]; ++j) below += a.A.id[a.perm[j]] < id;
+    a.off[s] = below;
+}
+
 // ---------------------------------------------------------------------------------- (B) scatter
 template <typename T>
 __global__ void __launch_bounds__(256) ped_scatter_kernel(PedArgs<T> a)
@@ -291,11 +334,6 @@ __global__ void __launch_bounds__(256) ped_occ_kernel(PedArgs<T> a)
     cellprev[d] = c;
 }
 
-// One candidate of the pair loop: adds A_s exp((2r - d)/B_s) (x_i - x_j)/d to (ax, ay) if 0 < d < R_int
-// (C24, C26).
-//   fp32: the difference and its squares on packed FADD2 / FFMA2; the squares carry +5e-31 each, so
-//   d2 >= 1e-30 > 0 and the agent itself or a coincident partner (d = 0, skipped by C26) needs no
-//   second compare: its force factor is finite and multiplies dx = dy = 0.  Two MUFU (rsqrt, ex2).
 // ---------------------------------------------------------------------------------- (P) pair loop
 // One candidate of the pair loop: adds A_s exp((2r - d)/B_s) (x_i - x_j)/d to (ax, ay) if 0 < d < R_int
 // (C24, C26).
@@ -483,7 +521,7 @@ template <typename T>
 struct TailArgs {
     Ctl *ctl;
     T *zs_tab[MAX_SLABS];            // bed of every row slab, pre-offset for the global cell index (8f-4)
-    int slab_rows, nx;
+    int slab_rows, nx, n_slabs;
     const int32_t *line_cells;
     int n_line, bags_per_cell_layer, n_layers;
     T layer_thickness;
@@ -618,7 +656,7 @@ __global__ void tail_kernel(TailArgs<T> a, int first)
                 l.bags += 1;
                 if (l.bags == a.bags_per_cell_layer) {
                     const int lc = a.line_cells[l.cursor];
-                    a.zs_tab[lc / a.nx / a.slab_rows][lc] += a.layer_thickness;
+                    a.zs_tab[min(lc / a.nx / a.slab_rows, a.n_slabs - 1)][lc] += a.layer_thickness;   // as SlabTab::of: the last slab may be the longer one
                     l.bags = 0; l.cursor += 1;
                     if (l.cursor == a.n_line) { l.layer += 1; l.cursor = 0; }
                     if (l.layer == a.n_layers) l.complete = 1;

@@ -41,22 +41,27 @@ def test_config1_fp64_slabs_bit_identical_per_cell_kernel(n_slabs):
     assert all(g.flood_variant() == 0 or g.flood_variant() == 4 for g in slabs.sims)
     for g in slabs.sims:
         g.set_flood_variant(0)
-    # pair forces are summed in the order of the counting sort's atomics, which is not reproducible
-    # between two runs: compare the flood bit for bit with the people -> flow coupling off ...
-    sc2 = S.make(1); sc2.couple_roughness = 0
-    one2 = binding.Sim(sc2); one2.set_flood_variant(0)
-    sl2 = binding.SlabSim(sc2, n_slabs)
-    for g in sl2.sims:
-        g.set_flood_variant(0)
+    # bins ordered by id (sim_set_deterministic): the pair forces are summed in the same order on the
+    # single handle and on the slabs, so with the people -> flow coupling ON the flood state and every
+    # pedestrian must agree bit for bit (agents walk across the cuts: Config 1 heads for one exit)
+    one.set_deterministic(True); slabs.sims[0].set_deterministic(True)
     for _ in range(4):
-        one2.step(25); sl2.step(25)
-        a, b = sl2.read_conserved(), one2.read_conserved()
+        one.step(25); slabs.step(25)
+        a, b = slabs.read_conserved(), one.read_conserved()
         for k in ("h", "qx", "qy"):
-            assert np.array_equal(a[k], b[k]), k
-        assert sl2.stats()["dt"] == one2.stats()["dt"]
-    # ... and with the coupling on against the oracle within the multi-step tolerances
+            assert np.array_equal(a[k].view(np.uint64), b[k].view(np.uint64)), k
+        assert slabs.stats()["dt"] == one.stats()["dt"]
+        pa, pb = slabs.read_peds(), one.read_peds()
+        for k in ("x", "y", "vx", "vy"):
+            assert np.array_equal(pa[k].view(np.uint64), pb[k].view(np.uint64)), k
+        for k in ("active", "fsm", "state", "cell"):
+            assert np.array_equal(pa[k], pb[k]), k
+        assert np.array_equal(slabs.read_occupancy(), one.read_occupancy())
+    rows = pb["cell"][pb["active"] == 1] // sc.nx
+    assert len({int(r) // slabs.cuts[0][1] for r in rows}) >= 2          # people on both sides of a cut
+    # ... and against the oracle within the multi-step tolerances
     o = oracle.Oracle(sc)
-    o.step(100); slabs.step(100)
+    o.step(100)
     sa, sb = slabs.stats(), o.stats()
     assert abs(sa["volume"] - sb["volume"]) <= 1e-10 * sb["volume"] and abs(sa["max_h"] - sb["max_h"]) <= 1e-9 * sb["max_h"]
     assert sa["hist"] == sb["hist"]
@@ -119,6 +124,27 @@ def test_link_validation():
         g.sims[0].step(1)
     with pytest.raises(binding.FloodpedError):
         g.sims[0].set_flood_variant(4)          # 64 columns: the strip sticks out of the grid, that path reads no halo row
+
+
+def test_attach_refuses_a_barrier_line_outside_the_first_slab():
+    """one process per slab: rank 0's tail kernel raises the bed after the step's only exchange, so a
+    deposit into another process's rows would race with that process's next flood kernel"""
+    import ctypes as C
+    from paper_1908_05232_b200.replicas import slab_cuts
+    sc = S.make(3, n=128, n_evac=50, n_resp=10)
+    line_rows = np.asarray(sc.line_cells) // sc.nx
+    for n_slabs, accepted in ((2, True), (8, False)):
+        cuts = slab_cuts(sc.ny, n_slabs)
+        assert (line_rows.max() < cuts[0][1]) == accepted
+        sims = [binding.Sim(sc, slab=cut, with_peds=(r == 0)) for r, cut in enumerate(cuts)]
+        descs = (binding.SlabDesc * n_slabs)()
+        for r, g in enumerate(sims):
+            g._chk(g._L.sim_slab_describe(g._h, C.byref(descs[r])))
+        rc = sims[0]._L.sim_slab_attach(sims[0]._h, 0, n_slabs, descs)
+        if accepted:
+            assert rc == 0
+        else:
+            assert rc == binding.SIM_EINVAL and b"first slab" in sims[0]._L.sim_last_error(sims[0]._h)
 
 
 def test_doors_and_trigger_on_slabs_match_the_oracle_step_by_step():
