@@ -74,3 +74,11 @@ def doors_box(n=24, slots=64, rate=0.5, target=1000, n_doors=3, **kw):
     sc.spawn_vpref_lo, sc.spawn_vpref_hi = 1.0, 1.4
     sc.pactive0 = np.zeros(slots, np.uint8)
     return sc
+
+
+def compass_scene(code, real_bits=64):
+    """one agent in the middle of a dry 64 x 64 hall whose navigation field holds `code` in every cell"""
+    n = 64
+    sc = box(n, n, dx=1.0, real_bits=real_bits, peds=dict(x=[32.5], y=[32.5], vpref=[1.3]), exit_cell=0, dt_max=0.2)
+    sc.nav_dir = np.full_like(sc.nav_dir, code)
+    return sc

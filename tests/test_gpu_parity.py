@@ -8,7 +8,7 @@ import pytest
 
 import oracle
 from paper_1908_05232_b200 import binding, scenarios as S
-from helpers import box, golden_rows
+from helpers import box, golden_rows, compass_scene
 from gpu_common import make_pair, sync, mixed, rounded, force_sum_tolerance
 
 pytestmark = pytest.mark.gpu
@@ -209,6 +209,33 @@ def test_binning_bit_exact(cfg, kw):
 
 
 # ------------------------------------------------------------------ pedestrians, single step
+
+@pytest.mark.parametrize("bits", [64, 32])
+def test_all_eight_navigation_codes_walk_their_compass_direction_on_the_gpu(bits):
+    """the kernel's own direction table (csrc/peds.cuh, step 3) against the closed-form free walk along
+    the hand-written compass direction, and against the oracle (tests/test_oracle_peds.py pins it the
+    same way): P:L83, SURVEY O3.3.  A diagonal that is not normalised fails by a factor sqrt 2."""
+    r = 1.0 / math.sqrt(2.0)
+    compass = {0: (1, 0), 1: (r, r), 2: (0, 1), 3: (-r, r), 4: (-1, 0), 5: (-r, -r), 6: (0, -1), 7: (r, -r)}
+    real = np.float64 if bits == 64 else np.float32
+    v0, tau, dt = float(real(1.3)), 0.5, float(real(0.2))
+    for code, (ex, ey) in compass.items():
+        sc = compass_scene(code, bits)
+        o = oracle.Oracle(sc); g = binding.Sim(sc)
+        for k in range(1, 13):
+            o.step(1); g.step(1)
+            a, b = g.read_peds(), o.read_peds()
+            s = v0 * (1 - (1 + dt / tau) ** (-k))
+            for key, want in (("vx", s * ex), ("vy", s * ey)):
+                assert abs(a[key][0] - want) <= TOL[bits] * v0, (code, k, key)
+                assert abs(a[key][0] - b[key][0]) <= TOL[bits] * v0, (code, k, key)
+            assert math.hypot(a["vx"][0], a["vy"][0]) <= v0
+            assert abs(a["x"][0] - b["x"][0]) <= TOL[bits] * 64 and abs(a["y"][0] - b["y"][0]) <= TOL[bits] * 64
+            assert a["cell"][0] == b["cell"][0]
+    g = binding.Sim(compass_scene(255, bits)); g.step(5)
+    a = g.read_peds()
+    assert a["vx"][0] == 0.0 and a["vy"][0] == 0.0 and a["x"][0] == 32.5 and a["y"][0] == 32.5
+
 
 def test_dense_crowd_single_step_fp64_and_fp32():
     rng = np.random.default_rng(9)

@@ -2,10 +2,11 @@
 import math
 
 import numpy as np
+import pytest
 
 import oracle
 from paper_1908_05232_b200 import scenarios as S
-from helpers import box, golden_rows
+from helpers import box, golden_rows, compass_scene
 
 
 # ------------------------------------------------------------------ HR, Table 1, roughness (paper)
@@ -152,6 +153,34 @@ def test_free_walk_relaxes_geometrically():
         assert abs(p["x"][0] - (x_prev + 0.2 * want)) < 1e-13
         x_prev = p["x"][0]
         assert p["state"][0] == 0 and p["active"][0] == 1
+
+
+@pytest.mark.parametrize("code", range(8))
+def test_all_eight_navigation_codes_walk_their_compass_direction_at_unit_norm(code):
+    """The eight codes of the navigation field (navigation agents hand out the direction to
+    the destination) are the compass points E, NE, N, NW, W, SW, S, SE, and the desired direction is a
+    UNIT vector: a diagonal walker is no faster than a straight one.  Closed form of the free walk
+    (backward-Euler relaxation) along e = (di, dj) / |(di, dj)|:
+        v_k = v0 (1 - (1 + dt/tau)^-k) e ,   |v_k| < v0 for every k, -> v0.
+    The expected direction is written out here by hand, not taken from any table of the code."""
+    r = 1.0 / math.sqrt(2.0)
+    compass = {0: (1, 0), 1: (r, r), 2: (0, 1), 3: (-r, r), 4: (-1, 0), 5: (-r, -r), 6: (0, -1), 7: (r, -r)}
+    ex, ey = compass[code]
+    o = oracle.Oracle(compass_scene(code))
+    x, y = 32.5, 32.5
+    for k in range(1, 25):
+        o.step(1)
+        p = o.read_peds()
+        s = 1.3 * (1 - (1 + 0.2 / 0.5) ** (-k))
+        assert abs(p["vx"][0] - s * ex) < 1e-14 and abs(p["vy"][0] - s * ey) < 1e-14, (code, k)
+        assert math.hypot(p["vx"][0], p["vy"][0]) < 1.3
+        x += 0.2 * s * ex; y += 0.2 * s * ey
+        assert abs(p["x"][0] - x) < 1e-12 and abs(p["y"][0] - y) < 1e-12
+    assert math.hypot(p["vx"][0], p["vy"][0]) > 1.3 * (1 - 1e-3)      # 1.4^-24 = 3e-4: at the desired speed, not above
+    # a code outside 0..7 (255 = none) gives no direction: the agent stays put
+    o = oracle.Oracle(compass_scene(255)); o.step(5)
+    p = o.read_peds()
+    assert p["vx"][0] == 0.0 and p["vy"][0] == 0.0 and p["x"][0] == 32.5 and p["y"][0] == 32.5
 
 
 def test_wet_speed_follows_table1_and_trapped_agents_stop():
